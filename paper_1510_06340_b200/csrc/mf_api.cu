@@ -1,0 +1,587 @@
+// mf_api.cu — the C ABI declared in include/mustaforce.h: context, device buffers, the RK stage driver.
+// Host logic only; every arithmetic step of the path runs in the kernels (mf_kernels.cu / mf_fused.cu).
+#include "../../include/mustaforce.h"
+#include "mf_kernels.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace mf;
+
+#ifdef MF_STRICT
+#define MF_VERSION_STR "mustaforce 0.1 sm_100a strict"
+#else
+#define MF_VERSION_STR "mustaforce 0.1 sm_100a"
+#endif
+
+struct mf_ctx {
+    Grid g;
+    Eos q;
+    int limiter, k, rk, predictor, nact;
+    double alpha;
+    Source src;
+    int path_req, path;
+    int dev, num_sms;
+    cudaStream_t own_stream, stream;
+    double* U[3];            // three state registers, 5*ncell doubles each (U^n, U_(1), U_(2)), component-major
+    int cur;                 // which register holds U^n
+    double* faces;           // staged path: 2*5*nact*next doubles
+    double* fluxes;          // staged path: 5*nact*next doubles
+    StepState* ds;
+    StepState* h_ds;         // pinned mirror
+    double* partials;        // totals: 5*nblocks doubles
+    double* h_partials;
+    int nblocks_tot;
+    long long launches;
+    std::string err;
+    // per-class CUDA-event timing (mf_profile)
+    int prof_on;
+    std::vector<cudaEvent_t> prof_ev;     // pairs: [2i] start, [2i+1] stop
+    std::vector<int> prof_cls;            // class of pair i
+    size_t prof_used;
+};
+
+namespace {
+
+thread_local std::string g_create_err;
+
+int fail(mf_ctx* c, int code, const std::string& msg) { if (c) c->err = msg; else g_create_err = msg; return code; }
+
+int cuda_fail(mf_ctx* c, cudaError_t e, const char* what)
+{
+    return fail(c, MF_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define MF_CUDA(c, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail((c), e_, #call); } while (0)
+
+CState5 cstate(const double* base, long long n) { CState5 s; for (int v = 0; v < 5; ++v) s.q[v] = base + v * n; return s; }
+State5 state(double* base, long long n) { State5 s; for (int v = 0; v < 5; ++v) s.q[v] = base + v * n; return s; }
+
+Faces faces_of(mf_ctx* c)
+{
+    Faces f; memset(&f, 0, sizeof(f));
+    long long slot = 0;
+    for (int d = 0; d < 3; ++d) {
+        if (!c->g.act[d]) continue;
+        for (int s = 0; s < 2; ++s) for (int v = 0; v < 5; ++v) f.f[d][s][v] = c->faces + (slot++) * c->g.next;
+    }
+    return f;
+}
+
+Fluxes fluxes_of(mf_ctx* c)
+{
+    Fluxes f; memset(&f, 0, sizeof(f));
+    long long slot = 0;
+    for (int d = 0; d < 3; ++d) {
+        if (!c->g.act[d]) continue;
+        for (int v = 0; v < 5; ++v) f.f[d][v] = c->fluxes + (slot++) * c->g.next;
+    }
+    return f;
+}
+
+void set_eos(Eos& q, double cs2)
+{
+    q.cs2 = cs2;
+    q.c1 = 1.0 + cs2;
+    q.c1sq = q.c1 * q.c1;
+    q.four_cs2 = 4.0 * cs2;
+    q.cs = std::sqrt(cs2);
+}
+
+int resolve_path(mf_ctx* c)
+{
+    if (c->path_req == MF_PATH_FUSED) { if (!fused_supported(c->g)) return MF_EINVAL; c->path = MF_PATH_FUSED; }
+    else if (c->path_req == MF_PATH_STAGED) c->path = MF_PATH_STAGED;
+    else c->path = fused_supported(c->g) ? MF_PATH_FUSED : MF_PATH_STAGED;
+    return MF_OK;
+}
+
+// RAII-free scope: record an event pair around the launches of one kernel class when profiling is on
+constexpr size_t PROF_MAX = 8192;
+int prof_begin(mf_ctx* c, int cls)
+{
+    if (!c->prof_on || c->prof_used >= PROF_MAX) return -1;
+    size_t i = c->prof_used;
+    if (c->prof_ev.size() < 2 * (i + 1)) {
+        cudaEvent_t a, b;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { cudaGetLastError(); return -1; }
+        c->prof_ev.push_back(a); c->prof_ev.push_back(b); c->prof_cls.push_back(cls);
+    }
+    c->prof_cls[i] = cls;
+    cudaEventRecord(c->prof_ev[2 * i], c->stream);
+    return (int)i;
+}
+void prof_end(mf_ctx* c, int slot)
+{
+    if (slot < 0) return;
+    cudaEventRecord(c->prof_ev[2 * slot + 1], c->stream);
+    c->prof_used = (size_t)slot + 1;
+}
+
+// staged path needs its scratch; allocate on first use so that the fused path keeps the footprint at 3 states
+int ensure_staged_buffers(mf_ctx* c)
+{
+    if (c->faces) return MF_OK;
+    size_t nf = (size_t)10 * c->nact * c->g.next, nx = (size_t)5 * c->nact * c->g.next;
+    if (cudaMalloc(&c->faces, nf * sizeof(double)) != cudaSuccess) { cudaGetLastError(); c->faces = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(face states) failed"); }
+    if (cudaMalloc(&c->fluxes, nx * sizeof(double)) != cudaSuccess) { cudaGetLastError(); cudaFree(c->faces); c->faces = nullptr; c->fluxes = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(fluxes) failed"); }
+    return MF_OK;
+}
+
+// One evaluation of  out = form(Ua, V, L(V) + S)  on the selected path.
+int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, double* out)
+{
+    const long long n = c->g.ncell;
+    if (c->path == MF_PATH_FUSED) {
+        int ps = prof_begin(c, 4);
+        c->launches += launch_fused_stage(c->g, c->q, c->limiter, c->predictor, c->k, cstate(V, n), sg, cstate(Ua, n), cstate(V, n),
+                                          state(out, n), c->src, c->ds, c->num_sms, c->stream);
+        prof_end(c, ps);
+    } else {
+        int rc = ensure_staged_buffers(c);
+        if (rc != MF_OK) return rc;
+        Faces fc = faces_of(c);
+        Fluxes fx = fluxes_of(c);
+        int ps = prof_begin(c, 1);
+        c->launches += launch_cell_stage(c->g, c->q, c->limiter, c->predictor, cstate(V, n), fc, c->ds, c->stream);
+        prof_end(c, ps);
+        ps = prof_begin(c, 2);
+        c->launches += launch_flux_stage(c->g, c->q, c->k, fc, fx, c->ds, c->stream);
+        prof_end(c, ps);
+        ps = prof_begin(c, 3);
+        c->launches += launch_combine(c->g, fx, sg, cstate(Ua, n), cstate(V, n), state(out, n), c->src, c->ds, c->stream);
+        prof_end(c, ps);
+    }
+    return MF_OK;
+}
+
+// RK2 (Eq.6 :103-105) / RK3 (Eq.7 :110-114); per-step scalars are already in c->ds.
+int run_step(mf_ctx* c)
+{
+    double* Un = c->U[c->cur];
+    double* Ra = c->U[(c->cur + 1) % 3];
+    double* Rb = c->U[(c->cur + 2) % 3];
+    int rc;
+    if (c->rk == 2) {
+        Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
+        Stage s2 = { 1, 0.5, 0.5, 1.0, 1.0 };
+        if ((rc = run_stage(c, Un, s1, Un, Ra)) != MF_OK) return rc;
+        if ((rc = run_stage(c, Ra, s2, Un, Rb)) != MF_OK) return rc;
+        c->cur = (c->cur + 2) % 3;
+    } else {
+        Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
+        Stage s2 = { 2, 0.75, 0.25, 0.25, 1.0 };
+        Stage s3 = { 2, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, 0.5 };
+        if ((rc = run_stage(c, Un, s1, Un, Ra)) != MF_OK) return rc;
+        if ((rc = run_stage(c, Ra, s2, Un, Rb)) != MF_OK) return rc;
+        if ((rc = run_stage(c, Rb, s3, Un, Ra)) != MF_OK) return rc;
+        c->cur = (c->cur + 1) % 3;
+    }
+    c->launches += launch_end_step(c->ds, c->stream);
+    return MF_OK;
+}
+
+int check_launch(mf_ctx* c)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch");
+    return MF_OK;
+}
+
+// synchronise and fetch the device-side step state into the pinned mirror
+int fetch_step_state(mf_ctx* c)
+{
+    MF_CUDA(c, cudaMemcpyAsync(c->h_ds, c->ds, sizeof(StepState), cudaMemcpyDeviceToHost, c->stream));
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->h_ds->status) return fail(c, MF_ESTATE, "a CFL reduction met a non-finite or superluminal (|M| > E) cell");
+    return MF_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+const char* mf_version(void) { return MF_VERSION_STR; }
+
+mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k_stages)
+{
+    const int n[3] = { nx, ny, nz };
+    for (int a = 0; a < 3; ++a)
+        if (n[a] < 1 || (n[a] > 1 && n[a] < 4)) { fail(nullptr, MF_EINVAL, "each extent must be 1 (inactive) or >= 4"); return nullptr; }
+    if (!(dx > 0.0)) { fail(nullptr, MF_EINVAL, "dx must be > 0"); return nullptr; }
+    if (eos != MF_EOS_CS2) { fail(nullptr, MF_EINVAL, "unknown eos"); return nullptr; }
+    if (limiter < 0 || limiter > MF_LIM_FIRST) { fail(nullptr, MF_EINVAL, "unknown limiter"); return nullptr; }
+    if (k_stages < 0 || k_stages > 8) { fail(nullptr, MF_EINVAL, "k_stages must be in 0..8"); return nullptr; }
+
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        fail(nullptr, MF_ECUDA, std::string("no CUDA device (there is no CPU fallback): ") + cudaGetErrorString(e));
+        return nullptr;
+    }
+    mf_ctx* c = new (std::nothrow) mf_ctx();
+    if (!c) { fail(nullptr, MF_ENOMEM, "host allocation failed"); return nullptr; }
+    memset(&c->g, 0, sizeof(c->g));
+    c->U[0] = c->U[1] = c->U[2] = nullptr; c->faces = c->fluxes = nullptr; c->ds = nullptr; c->h_ds = nullptr;
+    c->partials = nullptr; c->h_partials = nullptr; c->own_stream = nullptr; c->stream = nullptr;
+    cudaGetDevice(&c->dev);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, c->dev) != cudaSuccess || prop.major < 10) {
+        cudaGetLastError();
+        fail(nullptr, MF_ECUDA, "device is not sm_100 or newer (library is built for sm_100a only)");
+        delete c; return nullptr;
+    }
+    c->num_sms = prop.multiProcessorCount;
+    Grid& g = c->g;
+    c->nact = 0;
+    for (int a = 0; a < 3; ++a) {
+        g.n[a] = n[a]; g.act[a] = n[a] > 1; g.h[a] = g.act[a] ? 1 : 0; g.e[a] = n[a] + 2 * g.h[a];
+        c->nact += g.act[a];
+    }
+    g.periodic = 0;
+    g.ncell = (long long)nx * ny * nz;
+    g.next = (long long)g.e[0] * g.e[1] * g.e[2];
+    g.ns[0] = 1; g.ns[1] = nx; g.ns[2] = (long long)nx * ny;
+    g.es[0] = 1; g.es[1] = g.e[0]; g.es[2] = (long long)g.e[0] * g.e[1];
+    g.dx = dx;
+    set_eos(c->q, 1.0 / 3.0);
+    c->limiter = limiter; c->k = k_stages; c->rk = 2; c->predictor = 1;
+    c->alpha = c->nact > 0 ? (double)c->nact : 1.0;                 // A9
+    memset(&c->src, 0, sizeof(c->src));
+    c->path_req = MF_PATH_AUTO; c->cur = 0; c->launches = 0;
+    c->prof_on = 0; c->prof_used = 0;
+    resolve_path(c);
+    c->nblocks_tot = c->num_sms * 4;
+
+    bool ok = cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) == cudaSuccess;
+    c->stream = c->own_stream;
+    for (int r = 0; ok && r < 3; ++r) ok = cudaMalloc(&c->U[r], sizeof(double) * 5 * g.ncell) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->ds, sizeof(StepState)) == cudaSuccess;
+    ok = ok && cudaMallocHost(&c->h_ds, sizeof(StepState)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->partials, sizeof(double) * 5 * c->nblocks_tot) == cudaSuccess;
+    ok = ok && cudaMallocHost(&c->h_partials, sizeof(double) * 5 * c->nblocks_tot) == cudaSuccess;
+    if (ok) {
+        for (int r = 0; r < 3; ++r) cudaMemsetAsync(c->U[r], 0, sizeof(double) * 5 * g.ncell, c->stream);
+        c->launches += launch_reset(c->ds, c->stream);
+        ok = cudaStreamSynchronize(c->stream) == cudaSuccess;
+    }
+    if (!ok) {
+        cudaError_t le = cudaGetLastError();
+        fail(nullptr, MF_ENOMEM, std::string("device allocation failed: ") + cudaGetErrorString(le));
+        mf_destroy(c);
+        return nullptr;
+    }
+    return c;
+}
+
+void mf_destroy(mf_ctx* c)
+{
+    if (!c) return;
+    if (c->stream) cudaStreamSynchronize(c->stream);
+    for (int r = 0; r < 3; ++r) if (c->U[r]) cudaFree(c->U[r]);
+    if (c->faces) cudaFree(c->faces);
+    if (c->fluxes) cudaFree(c->fluxes);
+    if (c->ds) cudaFree(c->ds);
+    if (c->h_ds) cudaFreeHost(c->h_ds);
+    if (c->partials) cudaFree(c->partials);
+    if (c->h_partials) cudaFreeHost(c->h_partials);
+    if (c->own_stream) cudaStreamDestroy(c->own_stream);
+    for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
+    delete c;
+}
+
+const char* mf_last_error(mf_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+int mf_set_stream(mf_ctx* c, void* cuda_stream)
+{
+    if (!c) return MF_EINVAL;
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->stream = cuda_stream ? (cudaStream_t)cuda_stream : c->own_stream;
+    return MF_OK;
+}
+
+int mf_sync(mf_ctx* c)
+{
+    if (!c) return MF_EINVAL;
+    return fetch_step_state(c);
+}
+
+int mf_launch_count(mf_ctx* c, long long* launches)
+{
+    if (!c || !launches) return MF_EINVAL;
+    *launches = c->launches;
+    return MF_OK;
+}
+
+int mf_profile(mf_ctx* c, int on)
+{
+    if (!c) return MF_EINVAL;
+    c->prof_on = on ? 1 : 0;
+    return MF_OK;
+}
+
+int mf_profile_read(mf_ctx* c, double ms[MF_NCLASS], long long launches[MF_NCLASS])
+{
+    if (!c || !ms || !launches) return MF_EINVAL;
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < MF_NCLASS; ++k) { ms[k] = 0.0; launches[k] = 0; }
+    for (size_t i = 0; i < c->prof_used; ++i) {
+        float t = 0.f;
+        MF_CUDA(c, cudaEventElapsedTime(&t, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]));
+        ms[c->prof_cls[i]] += (double)t;
+        launches[c->prof_cls[i]] += 1;
+    }
+    c->prof_used = 0;
+    return MF_OK;
+}
+
+int mf_probe_fp64(double out[7])
+{
+    if (!out) return MF_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return MF_ECUDA; }
+    return probe_fp64(out) == 0 ? MF_OK : MF_ECUDA;
+}
+
+} // extern "C"
+
+// ============================================================================ state in / out, stepping, options
+namespace {
+
+int reset_after_set(mf_ctx* c)
+{
+    c->launches += launch_reset(c->ds, c->stream);
+    return check_launch(c);
+}
+
+int copy_in(mf_ctx* c, const double* const src[5], cudaMemcpyKind kind)
+{
+    c->cur = 0;
+    for (int v = 0; v < 5; ++v)
+        MF_CUDA(c, cudaMemcpyAsync(c->U[0] + v * c->g.ncell, src[v], sizeof(double) * c->g.ncell, kind, c->stream));
+    return MF_OK;
+}
+
+int copy_out(mf_ctx* c, const double* base, double* const dst[5], cudaMemcpyKind kind)
+{
+    for (int v = 0; v < 5; ++v)
+        MF_CUDA(c, cudaMemcpyAsync(dst[v], base + v * c->g.ncell, sizeof(double) * c->g.ncell, kind, c->stream));
+    return MF_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int mf_set_state(mf_ctx* c, const double* E, const double* Mx, const double* My, const double* Mz, const double* R)
+{
+    if (!c) return MF_EINVAL;
+    if (!E || !Mx || !My || !Mz || !R) return fail(c, MF_EINVAL, "null pointer");
+    const double* src[5] = { E, Mx, My, Mz, R };
+    int rc = copy_in(c, src, cudaMemcpyHostToDevice);
+    if (rc != MF_OK) return rc;
+    if ((rc = reset_after_set(c)) != MF_OK) return rc;
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MF_OK;
+}
+
+int mf_set_state_device(mf_ctx* c, const double* E, const double* Mx, const double* My, const double* Mz, const double* R)
+{
+    if (!c) return MF_EINVAL;
+    if (!E || !Mx || !My || !Mz || !R) return fail(c, MF_EINVAL, "null pointer");
+    const double* src[5] = { E, Mx, My, Mz, R };
+    int rc = copy_in(c, src, cudaMemcpyDeviceToDevice);
+    if (rc != MF_OK) return rc;
+    return reset_after_set(c);
+}
+
+int mf_get_state(mf_ctx* c, double* E, double* Mx, double* My, double* Mz, double* R)
+{
+    if (!c) return MF_EINVAL;
+    if (!E || !Mx || !My || !Mz || !R) return fail(c, MF_EINVAL, "null pointer");
+    double* dst[5] = { E, Mx, My, Mz, R };
+    int rc = copy_out(c, c->U[c->cur], dst, cudaMemcpyDeviceToHost);
+    if (rc != MF_OK) return rc;
+    return fetch_step_state(c);
+}
+
+int mf_get_state_device(mf_ctx* c, double* E, double* Mx, double* My, double* Mz, double* R)
+{
+    if (!c) return MF_EINVAL;
+    if (!E || !Mx || !My || !Mz || !R) return fail(c, MF_EINVAL, "null pointer");
+    double* dst[5] = { E, Mx, My, Mz, R };
+    int rc = copy_out(c, c->U[c->cur], dst, cudaMemcpyDeviceToDevice);
+    if (rc != MF_OK) return rc;
+    return fetch_step_state(c);
+}
+
+int mf_set_state_prim(mf_ctx* c, const double* e, const double* vx, const double* vy, const double* vz, const double* n)
+{
+    if (!c) return MF_EINVAL;
+    if (!e || !vx || !vy || !vz || !n) return fail(c, MF_EINVAL, "null pointer");
+    const double* src[5] = { e, vx, vy, vz, n };
+    int rc = copy_in(c, src, cudaMemcpyHostToDevice);
+    if (rc != MF_OK) return rc;
+    c->launches += launch_prim2con(c->g, c->q, state(c->U[0], c->g.ncell), c->stream);      // Eq.4 on the device
+    if ((rc = reset_after_set(c)) != MF_OK) return rc;
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MF_OK;
+}
+
+int mf_get_state_prim(mf_ctx* c, double* e, double* vx, double* vy, double* vz, double* n)
+{
+    if (!c) return MF_EINVAL;
+    if (!e || !vx || !vy || !vz || !n) return fail(c, MF_EINVAL, "null pointer");
+    double* scratch = c->U[(c->cur + 1) % 3];
+    c->launches += launch_con2prim(c->g, c->q, cstate(c->U[c->cur], c->g.ncell), state(scratch, c->g.ncell), c->stream);
+    int rc = check_launch(c);
+    if (rc != MF_OK) return rc;
+    double* dst[5] = { e, vx, vy, vz, n };
+    if ((rc = copy_out(c, scratch, dst, cudaMemcpyDeviceToHost)) != MF_OK) return rc;
+    return fetch_step_state(c);
+}
+
+int mf_step(mf_ctx* c, int n, double cfl)
+{
+    if (!c) return MF_EINVAL;
+    if (n < 0 || !(cfl > 0.0)) return fail(c, MF_EINVAL, "bad n or cfl");
+    for (int s = 0; s < n; ++s) {
+        int ps = prof_begin(c, 0);
+        c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->g.ncell), c->ds, c->num_sms, c->stream);   // a2, from U^n
+        prof_end(c, ps);
+        c->launches += launch_begin_step(c->ds, 0, cfl, c->g.dx, c->alpha, c->stream);
+        int rc = run_step(c);
+        if (rc != MF_OK) return rc;
+    }
+    return check_launch(c);
+}
+
+int mf_step_dt(mf_ctx* c, int n, double dt)
+{
+    if (!c) return MF_EINVAL;
+    if (n < 0 || !(dt > 0.0)) return fail(c, MF_EINVAL, "bad n or dt");
+    for (int s = 0; s < n; ++s) {
+        c->launches += launch_begin_step(c->ds, 1, dt, c->g.dx, c->alpha, c->stream);
+        int rc = run_step(c);
+        if (rc != MF_OK) return rc;
+    }
+    return check_launch(c);
+}
+
+int mf_eval_L(mf_ctx* c, double dt, double* L_E, double* L_Mx, double* L_My, double* L_Mz, double* L_R)
+{
+    if (!c) return MF_EINVAL;
+    if (!(dt > 0.0) || !L_E || !L_Mx || !L_My || !L_Mz || !L_R) return fail(c, MF_EINVAL, "bad dt or null pointer");
+    double* Un = c->U[c->cur];
+    double* scratch = c->U[(c->cur + 1) % 3];
+    c->launches += launch_begin_step(c->ds, 1, dt, c->g.dx, c->alpha, c->stream);
+    Stage sg = { 3, 0.0, 0.0, 0.0, 0.0 };
+    Source keep = c->src;
+    c->src.on = 0;
+    int rc = run_stage(c, Un, sg, Un, scratch);
+    c->src = keep;
+    if (rc != MF_OK) return rc;
+    if ((rc = check_launch(c)) != MF_OK) return rc;
+    double* dst[5] = { L_E, L_Mx, L_My, L_Mz, L_R };
+    if ((rc = copy_out(c, scratch, dst, cudaMemcpyDeviceToHost)) != MF_OK) return rc;
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MF_OK;
+}
+
+int mf_conserved_totals(mf_ctx* c, double out[5])
+{
+    if (!c || !out) return MF_EINVAL;
+    c->launches += launch_totals(c->g, cstate(c->U[c->cur], c->g.ncell), c->partials, c->nblocks_tot, c->stream);
+    int rc = check_launch(c);
+    if (rc != MF_OK) return rc;
+    MF_CUDA(c, cudaMemcpyAsync(c->h_partials, c->partials, sizeof(double) * 5 * c->nblocks_tot, cudaMemcpyDeviceToHost, c->stream));
+    rc = fetch_step_state(c);
+    double vol = 1.0;
+    for (int a = 0; a < 3; ++a) if (c->g.act[a]) vol *= c->g.dx;
+    for (int v = 0; v < 5; ++v) {
+        long double acc = 0.0L;
+        for (int b = 0; b < c->nblocks_tot; ++b) acc += (long double)c->h_partials[v * c->nblocks_tot + b];
+        out[v] = (double)(acc * (long double)vol);
+    }
+    return rc;
+}
+
+int mf_get_time(mf_ctx* c, double* t, double* last_dt, long long* steps)
+{
+    if (!c) return MF_EINVAL;
+    int rc = fetch_step_state(c);
+    if (t) *t = c->h_ds->t;
+    if (last_dt) *last_dt = c->h_ds->dt;
+    if (steps) *steps = c->h_ds->steps;
+    return rc;
+}
+
+int mf_max_signal_speed(mf_ctx* c, double* smax)
+{
+    if (!c || !smax) return MF_EINVAL;
+    c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->g.ncell), c->ds, c->num_sms, c->stream);
+    int rc = check_launch(c);
+    if (rc != MF_OK) return rc;
+    rc = fetch_step_state(c);
+    unsigned long long bits = c->h_ds->smax_bits;
+    memcpy(smax, &bits, sizeof(double));
+    // leave the accumulator empty for the next reduction
+    cudaMemsetAsync(&c->ds->smax_bits, 0, sizeof(unsigned long long), c->stream);
+    return rc;
+}
+
+int mf_set_rk(mf_ctx* c, int order)
+{
+    if (!c) return MF_EINVAL;
+    if (order != 2 && order != 3) return fail(c, MF_EINVAL, "rk order must be 2 or 3");
+    c->rk = order; return MF_OK;
+}
+int mf_set_boundary(mf_ctx* c, int bc)
+{
+    if (!c) return MF_EINVAL;
+    if (bc != MF_BC_OUTFLOW && bc != MF_BC_PERIODIC) return fail(c, MF_EINVAL, "unknown boundary condition");
+    c->g.periodic = bc == MF_BC_PERIODIC; return MF_OK;
+}
+int mf_set_cs2(mf_ctx* c, double cs2)
+{
+    if (!c) return MF_EINVAL;
+    if (!(cs2 > 0.0) || !(cs2 < 1.0)) return fail(c, MF_EINVAL, "cs2 must be in (0,1)");
+    set_eos(c->q, cs2); return MF_OK;
+}
+int mf_set_predictor(mf_ctx* c, int on) { if (!c) return MF_EINVAL; c->predictor = on ? 1 : 0; return MF_OK; }
+int mf_set_alpha(mf_ctx* c, double alpha)
+{
+    if (!c) return MF_EINVAL;
+    if (!(alpha > 0.0)) return fail(c, MF_EINVAL, "alpha must be > 0");
+    c->alpha = alpha; return MF_OK;
+}
+int mf_set_jet_source(mf_ctx* c, double dEdx, double sigma, double x0, double y0, double z0)
+{
+    if (!c) return MF_EINVAL;
+    if (dEdx != 0.0 && !(sigma > 0.0)) return fail(c, MF_EINVAL, "sigma must be > 0");
+    const double PI = 3.14159265358979323846;
+    double s2 = sigma > 0.0 ? sigma * sigma : 1.0;
+    c->src.dEdx = dEdx;
+    c->src.norm = 1.0 / std::pow(2.0 * PI * s2, 1.5);
+    c->src.inv_two_s2 = 1.0 / (2.0 * s2);
+    c->src.x0 = x0; c->src.y0 = y0; c->src.z0 = z0;
+    c->src.on = dEdx != 0.0;
+    return MF_OK;
+}
+int mf_set_path(mf_ctx* c, int path)
+{
+    if (!c) return MF_EINVAL;
+    if (path < MF_PATH_AUTO || path > MF_PATH_FUSED) return fail(c, MF_EINVAL, "unknown path");
+    int keep = c->path_req;
+    c->path_req = path;
+    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "the fused path does not support this configuration"); }
+    return MF_OK;
+}
+int mf_get_path(mf_ctx* c, int* path) { if (!c || !path) return MF_EINVAL; *path = c->path; return MF_OK; }
+
+} // extern "C"

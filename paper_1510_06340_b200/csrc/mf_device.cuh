@@ -1,0 +1,127 @@
+// mf_device.cuh — per-cell / per-interface device arithmetic of the MUSTA-FORCE step (fp64, sm_100a).
+// Everything here lives in registers; the kernels in mf_kernels.cu decide where operands come from.
+// Citations are PAPER.md lines; readings A1..A17 are listed in DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace mf {
+
+constexpr double E_VACUUM = 1e-12;        // A12(i)
+constexpr double V_CAP    = 1.0 - 1e-10;  // A12(ii)
+
+enum Limiter { LIM_NONE = 0, LIM_MINMOD = 1, LIM_SUPERBEE = 2, LIM_VANALBADA = 3, LIM_VANLEER = 4, LIM_MC = 5, LIM_FIRST = 6 };
+
+// p = cs2*e constants, computed once on the host in the order of reading A16
+struct Eos {
+    double cs2;
+    double c1;      // 1 + cs2
+    double c1sq;    // c1*c1
+    double four_cs2;
+    double cs;      // sqrt(cs2)
+};
+
+// ---- Eq.14-21 in two-argument form (A6): a = U_i - U_{i-1}, b = U_{i+1} - U_i; returns the limited slope
+template <int LIM>
+__device__ __forceinline__ double slope2(double a, double b)
+{
+    if (LIM == LIM_NONE) return 0.5 * (a + b);                                     // Eq.14 :177
+    if (LIM == LIM_FIRST) return 0.0;
+    if (LIM == LIM_VANALBADA) {                                                    // Eq.20 :205 as printed (A7)
+        double den = a * a + b * b;
+        return den > 0.0 ? (a * b) * (a + b) / den : 0.0;
+    }
+    double ab = a * b;
+    if (LIM == LIM_VANLEER) return ab > 0.0 ? 2.0 * ab / (a + b) : 0.0;            // Eq.21 :207
+    double fa = fabs(a), fb = fabs(b), m;
+    if (LIM == LIM_MINMOD) m = fmin(fa, fb);                                       // Eq.18 :201
+    else if (LIM == LIM_SUPERBEE) m = fmax(fmin(2.0 * fb, fa), fmin(fb, 2.0 * fa));// Eq.19 :203
+    else m = fmin(fmin(2.0 * fa, 2.0 * fb), 0.5 * fabs(a + b));                    // MC (A8)
+    m = copysign(m, a);
+    return ab > 0.0 ? m : 0.0;
+}
+
+// ---- Eq.23 for p = cs2*e in closed form with the admissibility guard A12.  :227-234
+// Returns the three velocity components and the pressure.
+__device__ __forceinline__ void velocity_pressure(const Eos& q, double E, double Mx, double My, double Mz,
+                                                  double& vx, double& vy, double& vz, double& e, double& p)
+{
+    double M2 = Mx * Mx + My * My + Mz * Mz;
+    double cap = V_CAP * E;
+    if (!(E > E_VACUUM)) {                        // vacuum (or NaN): v = 0, p = 0
+        bool nan = E != E;
+        vx = vy = vz = nan ? E : 0.0; e = E; p = nan ? E : 0.0;
+        return;
+    }
+    if (M2 > cap * cap) {                         // superluminal: rescale M to |M| = V_CAP*E, keep direction
+        double s = cap / sqrt(M2);
+        Mx *= s; My *= s; Mz *= s;
+        M2 = Mx * Mx + My * My + Mz * Mz;
+    }
+    double Q = sqrt(q.c1sq * E * E - q.four_cs2 * M2);
+    double inv = 2.0 / (q.c1 * E + Q);
+    vx = Mx * inv; vy = My * inv; vz = Mz * inv;
+    e = E - (Mx * vx + My * vy + Mz * vz);
+    p = q.cs2 * e;
+}
+
+// ---- Eq.3 :53-59: F_d(U) = ((E+p)v_d, M_j v_d + p delta_jd, R v_d)
+template <int D>
+__device__ __forceinline__ void flux_d(const Eos& q, const double (&U)[5], double (&F)[5])
+{
+    double vx, vy, vz, e, p;
+    velocity_pressure(q, U[0], U[1], U[2], U[3], vx, vy, vz, e, p);
+    double vd = D == 0 ? vx : (D == 1 ? vy : vz);
+    F[0] = (U[0] + p) * vd;
+    F[1] = U[1] * vd;
+    F[2] = U[2] * vd;
+    F[3] = U[3] * vd;
+    F[1 + D] += p;
+    F[4] = U[4] * vd;
+}
+
+// ---- MUSTA_k with FORCE-alpha, steps 1-5 :123-135, Eq.8-11 :130-149 (A1: Richtmyer state uses the flux difference)
+// A, B are U_L^(0), U_R^(0) on entry and are overwritten.
+template <int D>
+__device__ __forceinline__ void musta_flux(const Eos& q, int k, double lam, double c_lw, double c_lf,
+                                           double (&A)[5], double (&B)[5], double (&F)[5])
+{
+    for (int l = 0;; ++l) {
+        double FA[5], FB[5], W[5];
+        flux_d<D>(q, A, FA);
+        flux_d<D>(q, B, FB);
+#pragma unroll
+        for (int c = 0; c < 5; ++c) W[c] = 0.5 * (A[c] + B[c]) - c_lw * (FB[c] - FA[c]);      // Eq.10
+        flux_d<D>(q, W, F);                                                                   // F^lw
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+            double Flf = 0.5 * (FA[c] + FB[c]) - c_lf * (B[c] - A[c]);                        // Eq.11
+            F[c] = 0.5 * (F[c] + Flf);                                                        // Eq.9
+        }
+        if (l == k) break;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {                                                         // Eq.8
+            A[c] = A[c] - lam * (F[c] - FA[c]);
+            B[c] = B[c] - lam * (FB[c] - F[c]);
+        }
+    }
+}
+
+// ---- a2: local signal speed (|v|+cs)/(1+|v|cs) (A10) and the state check behind MF_ESTATE
+__device__ __forceinline__ double signal_speed(const Eos& q, double E, double Mx, double My, double Mz, double R, int& bad)
+{
+    bool finite = isfinite(E) && isfinite(Mx) && isfinite(My) && isfinite(Mz) && isfinite(R);
+    if (!finite) { bad = 1; return 0.0; }
+    if (E > E_VACUUM && Mx * Mx + My * My + Mz * Mz > E * E) bad = 1;
+    double vx, vy, vz, e, p;
+    velocity_pressure(q, E, Mx, My, Mz, vx, vy, vz, e, p);
+    double av = sqrt(vx * vx + vy * vy + vz * vz);
+    return (av + q.cs) / (1.0 + av * q.cs);
+}
+
+__device__ __forceinline__ int bc_index(int i, int n, int periodic)
+{
+    if (periodic) { i = i < 0 ? i + n : i; return i >= n ? i - n : i; }     // |offset| <= 2 < n
+    return min(max(i, 0), n - 1);
+}
+
+} // namespace mf

@@ -1,0 +1,343 @@
+// mf_kernels.cu — staged path (MF_PATH_STAGED) and the small kernels every path shares:
+// CFL reduction (a2), per-step scalars, cell stage (a3+a4), interface flux stage (a5+a6), combine (a7+a8),
+// prim<->con conversions, totals.  Boundary handling (a1) is index mapping in the loads: no stored ghosts.
+#include "mf_kernels.h"
+
+namespace mf {
+
+constexpr int TPB = 256;
+
+static inline unsigned int blocks_for(long long n, int tpb) { return (unsigned int)((n + tpb - 1) / tpb); }
+
+// =========================================================================== a2: CFL reduction
+__global__ void __launch_bounds__(TPB) k_cfl(Grid g, Eos q, CState5 U, StepState* ds)
+{
+    double smax = 0.0;
+    int bad = 0;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < g.ncell; o += stride) {
+        double s = signal_speed(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], U.q[4][o], bad);
+        smax = fmax(smax, s);
+    }
+    // warp shuffle max, then one value per warp through shared memory, then one atomic per block
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, off));
+        bad |= __shfl_xor_sync(0xffffffffu, bad, off);
+    }
+    __shared__ double s_max[TPB / 32];
+    __shared__ int s_bad[TPB / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) { s_max[warp] = smax; s_bad[warp] = bad; }
+    __syncthreads();
+    if (warp == 0) {
+        smax = lane < TPB / 32 ? s_max[lane] : 0.0;
+        bad = lane < TPB / 32 ? s_bad[lane] : 0;
+#pragma unroll
+        for (int off = 4; off > 0; off >>= 1) {
+            smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, off));
+            bad |= __shfl_xor_sync(0xffffffffu, bad, off);
+        }
+        if (lane == 0) {
+            atomicMax(&ds->smax_bits, (unsigned long long)__double_as_longlong(smax));   // smax >= 0: bit order == value order
+            if (bad) atomicOr(&ds->status, 1);
+        }
+    }
+}
+
+int launch_cfl(const Grid& g, const Eos& q, CState5 U, StepState* ds, int num_sms, cudaStream_t st)
+{
+    unsigned int nb = blocks_for(g.ncell, TPB);
+    unsigned int cap = (unsigned int)num_sms * 8u;
+    if (nb > cap) nb = cap;
+    k_cfl<<<nb, TPB, 0, st>>>(g, q, U, ds);
+    return 1;
+}
+
+// =========================================================================== per-step scalars
+__global__ void k_begin_step(StepState* ds, int mode, double value, double dx, double alpha)
+{
+    double dt;
+    if (mode == 0) {
+        double smax = __longlong_as_double((long long)ds->smax_bits);
+        dt = value * dx / smax;                                   // A10
+    } else {
+        dt = value;
+    }
+    double lam = dt / dx;
+    ds->dt = dt;
+    ds->lam = lam;
+    ds->hl = 0.5 * lam;
+    ds->c_lw = 0.5 * alpha * lam;                                 // A16: computed once per step, in this order
+    ds->c_lf = 0.5 / (alpha * lam);
+    ds->smax_bits = 0ull;
+}
+
+__global__ void k_end_step(StepState* ds)
+{
+    ds->t = ds->t + ds->dt;
+    ds->steps += 1;
+}
+
+__global__ void k_reset(StepState* ds)
+{
+    ds->t = 0.0; ds->dt = 0.0; ds->lam = 0.0; ds->hl = 0.0; ds->c_lw = 0.0; ds->c_lf = 0.0;
+    ds->smax_bits = 0ull; ds->status = 0; ds->pad = 0; ds->steps = 0;
+}
+
+int launch_begin_step(StepState* ds, int mode, double value, double dx, double alpha, cudaStream_t st)
+{
+    k_begin_step<<<1, 1, 0, st>>>(ds, mode, value, dx, alpha);
+    return 1;
+}
+int launch_end_step(StepState* ds, cudaStream_t st) { k_end_step<<<1, 1, 0, st>>>(ds); return 1; }
+int launch_reset(StepState* ds, cudaStream_t st) { k_reset<<<1, 1, 0, st>>>(ds); return 1; }
+
+// =========================================================================== a3 + a4: cell stage
+// One thread per cell of the extended region (interior + 1 layer on every active axis).
+template <int LIM>
+__global__ void __launch_bounds__(TPB) k_cell_stage(Grid g, Eos q, int predictor, CState5 V, Faces fc, const StepState* ds)
+{
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= g.next) return;
+    int ie = (int)(p % g.e[0]);
+    long long r = p / g.e[0];
+    int je = (int)(r % g.e[1]);
+    int ke = (int)(r / g.e[1]);
+    const int c[3] = { ie - g.h[0], je - g.h[1], ke - g.h[2] };             // interior coordinates, may be -1 or n
+    int cc[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) cc[a] = g.act[a] ? bc_index(c[a], g.n[a], g.periodic) : 0;
+    const long long o0 = cc[0] * g.ns[0] + cc[1] * g.ns[1] + cc[2] * g.ns[2];
+    double U0[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) U0[v] = V.q[v][o0];
+
+    double UL[3][5], UR[3][5];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        if (!g.act[d]) continue;
+        const long long om = o0 + (long long)(bc_index(c[d] - 1, g.n[d], g.periodic) - cc[d]) * g.ns[d];
+        const long long op = o0 + (long long)(bc_index(c[d] + 1, g.n[d], g.periodic) - cc[d]) * g.ns[d];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+            double a = U0[v] - V.q[v][om];
+            double b = V.q[v][op] - U0[v];
+            double s = slope2<LIM>(a, b);                                  // Eq.15-17
+            UL[d][v] = U0[v] - 0.5 * s;                                    // Eq.12 :161
+            UR[d][v] = U0[v] + 0.5 * s;
+        }
+    }
+    if (predictor) {                                                        // Eq.13 (A3)
+        const double hl = ds->hl;
+        double delta[5];
+        bool first = true;
+        double Fl[5], Fr[5];
+        if (g.act[0]) {
+            flux_d<0>(q, UL[0], Fl); flux_d<0>(q, UR[0], Fr);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) delta[v] = hl * (Fl[v] - Fr[v]);
+            first = false;
+        }
+        if (g.act[1]) {
+            flux_d<1>(q, UL[1], Fl); flux_d<1>(q, UR[1], Fr);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { double t = hl * (Fl[v] - Fr[v]); delta[v] = first ? t : delta[v] + t; }
+            first = false;
+        }
+        if (g.act[2]) {
+            flux_d<2>(q, UL[2], Fl); flux_d<2>(q, UR[2], Fr);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { double t = hl * (Fl[v] - Fr[v]); delta[v] = first ? t : delta[v] + t; }
+        }
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            if (!g.act[d]) continue;
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { UL[d][v] += delta[v]; UR[d][v] += delta[v]; }
+        }
+    }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        if (!g.act[d]) continue;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) { fc.f[d][0][v][p] = UL[d][v]; fc.f[d][1][v][p] = UR[d][v]; }
+    }
+}
+
+int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, CState5 V, Faces fc, const StepState* ds, cudaStream_t st)
+{
+    unsigned int nb = blocks_for(g.next, TPB);
+    switch (limiter) {
+#define MF_CASE(L) case L: k_cell_stage<L><<<nb, TPB, 0, st>>>(g, q, predictor, V, fc, ds); break;
+        MF_CASE(LIM_NONE) MF_CASE(LIM_MINMOD) MF_CASE(LIM_SUPERBEE) MF_CASE(LIM_VANALBADA) MF_CASE(LIM_VANLEER) MF_CASE(LIM_MC) MF_CASE(LIM_FIRST)
+#undef MF_CASE
+    default: return 0;
+    }
+    return 1;
+}
+
+// =========================================================================== a5 + a6: interface fluxes
+// One thread per interface between cell c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
+template <int D>
+__global__ void __launch_bounds__(TPB) k_flux_stage(Grid g, Eos q, int k, Faces fc, Fluxes fx, const StepState* ds)
+{
+    int m[3] = { g.n[0], g.n[1], g.n[2] };
+    m[D] += 1;
+    const long long total = (long long)m[0] * m[1] * m[2];
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= total) return;
+    int c[3];
+    c[0] = (int)(t % m[0]);
+    long long r = t / m[0];
+    c[1] = (int)(r % m[1]);
+    c[2] = (int)(r / m[1]);
+    c[D] -= 1;
+    const long long p = (c[0] + g.h[0]) * g.es[0] + (c[1] + g.h[1]) * g.es[1] + (c[2] + g.h[2]) * g.es[2];
+    double A[5], B[5], F[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) { A[v] = fc.f[D][1][v][p]; B[v] = fc.f[D][0][v][p + g.es[D]]; }   // A2 :173
+    musta_flux<D>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) fx.f[D][v][p] = F[v];
+}
+
+int launch_flux_stage(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx, const StepState* ds, cudaStream_t st)
+{
+    int launches = 0;
+    for (int d = 0; d < 3; ++d) {
+        if (!g.act[d]) continue;
+        long long total = 1;
+        for (int a = 0; a < 3; ++a) total *= (a == d) ? g.n[a] + 1 : g.n[a];
+        unsigned int nb = blocks_for(total, TPB);
+        if (d == 0) k_flux_stage<0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds);
+        if (d == 1) k_flux_stage<1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds);
+        if (d == 2) k_flux_stage<2><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds);
+        ++launches;
+    }
+    return launches;
+}
+
+// =========================================================================== a7 + a8: divergence, source, RK combine
+__device__ __forceinline__ double jet_source(const Grid& g, const Source& s, int i, int j, int k, double t)
+{
+    double x = (i + 0.5 - g.n[0] / 2.0) * g.dx - (s.x0 + t);
+    double y = (j + 0.5 - g.n[1] / 2.0) * g.dx - s.y0;
+    double z = (k + 0.5 - g.n[2] / 2.0) * g.dx - s.z0;
+    double r2 = x * x + y * y + z * z;
+    double arg = -r2 * s.inv_two_s2;
+#ifndef MF_STRICT
+    if (arg < -745.0) return 0.0;            // exp underflows to 0 in fp64 anyway
+#endif
+    return s.dEdx * s.norm * exp(arg);
+}
+
+__device__ __forceinline__ double rk_form(const Stage& sg, double ua, double ub, double dt, double L)
+{
+    if (sg.form == 0) return ua + dt * L;                          // U + dt L            (Eq.6/7 first line)
+    if (sg.form == 1) return 0.5 * (ua + ub + dt * L);             // Eq.6 second line :105
+    if (sg.form == 2) return sg.ca * ua + sg.cb * ub + (sg.cdt * dt) * L;   // Eq.7 lines 2, 3 :112-114
+    return L;                                                      // form 3: L itself (mf_eval_L)
+}
+
+__global__ void __launch_bounds__(TPB) k_combine(Grid g, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, const StepState* ds)
+{
+    const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= g.ncell) return;
+    int i = (int)(o % g.n[0]);
+    long long r = o / g.n[0];
+    int j = (int)(r % g.n[1]);
+    int k = (int)(r / g.n[1]);
+    const long long p = (i + g.h[0]) * g.es[0] + (j + g.h[1]) * g.es[1] + (k + g.h[2]) * g.es[2];
+    const double dt = ds->dt;
+    double S = 0.0;
+    if (src.on) S = jet_source(g, src, i, j, k, ds->t + sg.ts * dt);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+        double acc = 0.0;
+        bool first = true;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            if (!g.act[d]) continue;
+            double diff = fx.f[d][v][p] - fx.f[d][v][p - g.es[d]];
+            acc = first ? diff : acc + diff;
+            first = false;
+        }
+        double L = -acc / g.dx;                                    // Eq.1 :43
+        if (src.on && v < 2) L = L + S;
+        double ua = sg.form == 3 ? 0.0 : Ua.q[v][o];
+        double ub = (sg.form == 1 || sg.form == 2) ? Ub.q[v][o] : 0.0;
+        out.q[v][o] = rk_form(sg, ua, ub, dt, L);
+    }
+}
+
+int launch_combine(const Grid& g, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, const StepState* ds, cudaStream_t st)
+{
+    k_combine<<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, fx, sg, Ua, Ub, out, src, ds);
+    return 1;
+}
+
+// =========================================================================== conversions
+__global__ void __launch_bounds__(TPB) k_prim2con(Grid g, Eos q, State5 U)
+{
+    const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= g.ncell) return;
+    double e = U.q[0][o], vx = U.q[1][o], vy = U.q[2][o], vz = U.q[3][o], n = U.q[4][o];
+    double p = q.cs2 * e;                                          // Eq.4 :63-67
+    double g2 = 1.0 / (1.0 - (vx * vx + vy * vy + vz * vz));
+    double w = (e + p) * g2;
+    U.q[0][o] = w - p; U.q[1][o] = w * vx; U.q[2][o] = w * vy; U.q[3][o] = w * vz; U.q[4][o] = n * sqrt(g2);
+}
+
+__global__ void __launch_bounds__(TPB) k_con2prim(Grid g, Eos q, CState5 U, State5 P)
+{
+    const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= g.ncell) return;
+    double vx, vy, vz, e, p;
+    velocity_pressure(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], vx, vy, vz, e, p);
+    P.q[0][o] = e; P.q[1][o] = vx; P.q[2][o] = vy; P.q[3][o] = vz;
+    P.q[4][o] = U.q[4][o] * sqrt(1.0 - (vx * vx + vy * vy + vz * vz));   // n = R sqrt(1-v^2), Eq.23
+}
+
+int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st)
+{
+    k_prim2con<<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U);
+    return 1;
+}
+int launch_con2prim(const Grid& g, const Eos& q, CState5 U, State5 P, cudaStream_t st)
+{
+    k_con2prim<<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U, P);
+    return 1;
+}
+
+// =========================================================================== totals: per-block partial sums (host adds them in long double)
+__global__ void __launch_bounds__(TPB) k_totals(Grid g, CState5 U, double* partials)
+{
+    double acc[5] = { 0, 0, 0, 0, 0 };
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < g.ncell; o += stride)
+#pragma unroll
+        for (int v = 0; v < 5; ++v) acc[v] += U.q[v][o];
+    __shared__ double s[5][TPB / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) acc[v] += __shfl_xor_sync(0xffffffffu, acc[v], off);
+        if (lane == 0) s[v][warp] = acc[v];
+    }
+    __syncthreads();
+    if (threadIdx.x < 5) {
+        double t = 0.0;
+        for (int w = 0; w < TPB / 32; ++w) t += s[threadIdx.x][w];
+        partials[(long long)threadIdx.x * gridDim.x + blockIdx.x] = t;
+    }
+}
+
+int launch_totals(const Grid& g, CState5 U, double* partials, int nblocks, cudaStream_t st)
+{
+    k_totals<<<nblocks, TPB, 0, st>>>(g, U, partials);
+    return 1;
+}
+
+} // namespace mf

@@ -1,0 +1,33 @@
+// mf_kernels.h — launch wrappers of the CUDA kernels (defined in mf_kernels.cu, mf_fused.cu, mf_probe.cu).
+// Each wrapper enqueues on `st` and returns the number of kernel launches it issued.
+#pragma once
+#include "mf_types.h"
+
+namespace mf {
+
+// a2: CFL reduction of `U` into ds->smax_bits / ds->status (accumulator must have been reset by begin_step of the previous step or by reset_smax)
+int launch_cfl(const Grid& g, const Eos& q, CState5 U, StepState* ds, int num_sms, cudaStream_t st);
+// per-step scalars on the device: mode 0: dt = value*dx/smax (cfl), mode 1: dt = value (fixed); resets the smax accumulator
+int launch_begin_step(StepState* ds, int mode, double value, double dx, double alpha, cudaStream_t st);
+int launch_end_step(StepState* ds, cudaStream_t st);
+int launch_reset(StepState* ds, cudaStream_t st);
+
+// ---- staged path (MF_PATH_STAGED): a3+a4, a5, a7(+a8) as three kernels, face states and fluxes through HBM
+int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, CState5 V, Faces fc, const StepState* ds, cudaStream_t st);
+int launch_flux_stage(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx, const StepState* ds, cudaStream_t st);
+int launch_combine(const Grid& g, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, const StepState* ds, cudaStream_t st);
+
+// ---- fused path (MF_PATH_FUSED): one kernel per RK stage
+bool fused_supported(const Grid& g);
+int launch_fused_stage(const Grid& g, const Eos& q, int limiter, int predictor, int k, CState5 V, Stage sg, CState5 Ua, CState5 Ub,
+                       State5 out, Source src, const StepState* ds, int num_sms, cudaStream_t st);
+
+// ---- conversions and reductions
+int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st);          // in place: (e,v,n) -> (E,M,R), Eq.4
+int launch_con2prim(const Grid& g, const Eos& q, CState5 U, State5 P, cudaStream_t st); // Eq.23
+int launch_totals(const Grid& g, CState5 U, double* partials /* 5*nblocks */, int nblocks, cudaStream_t st);
+
+// ---- FP64 pipe micro-benchmarks (mf_probe_fp64)
+int probe_fp64(double out[7]);
+
+} // namespace mf

@@ -1,0 +1,63 @@
+// mf_types.h — plain structs shared by the host API (mf_api.cu) and the kernels (mf_kernels.cu).
+#pragma once
+#include <cuda_runtime.h>
+#include "mf_device.cuh"
+
+namespace mf {
+
+// Grid geometry, passed to kernels by value.
+struct Grid {
+    int n[3];          // interior extents (x, y, z)
+    int h[3];          // 1 on active axes, else 0: the ghost layer the face states are needed on
+    int e[3];          // n + 2h: extents of the "extended" layout that holds face states and fluxes
+    int act[3];
+    int periodic;
+    long long ncell;   // n0*n1*n2
+    long long next;    // e0*e1*e2
+    long long ns[3];   // strides of the interior layout
+    long long es[3];   // strides of the extended layout
+    double dx;
+};
+
+// Per-step scalars that live in device memory so that a step never needs the host (A10).
+struct StepState {
+    double t;                       // simulation time at the start of the current step
+    double dt;                      // this step's dt (same in every RK stage, A4)
+    double lam;                     // dt/dx
+    double hl;                      // 0.5*lam               (Eq.13)
+    double c_lw;                    // 0.5*alpha*lam         (Eq.10)
+    double c_lf;                    // 0.5/(alpha*lam)       (Eq.11)
+    unsigned long long smax_bits;   // atomicMax target: bit image of a non-negative double
+    int status;                     // sticky: 1 = bad state seen by a CFL reduction
+    int pad;
+    long long steps;
+};
+
+struct Source {
+    double dEdx, norm, inv_two_s2, x0, y0, z0;   // S = dEdx*norm*exp(-r^2*inv_two_s2)
+    int on;
+};
+
+// One conserved state: five component arrays
+struct State5 {
+    double* q[5];
+};
+struct CState5 {
+    const double* q[5];
+};
+
+// Face states of the staged path: [d][side][component] arrays in the extended layout, and interface fluxes [d][component]
+struct Faces {
+    double* f[3][2][5];
+};
+struct Fluxes {
+    double* f[3][5];
+};
+
+// RK stage description (Eq.6 / Eq.7): out = form(Ua, Ub, L + S(t + ts*dt))
+struct Stage {
+    int form;        // 0: Ua + dt*L   1: 0.5*(Ua + Ub + dt*L)   2: ca*Ua + cb*Ub + (cdt*dt)*L
+    double ca, cb, cdt, ts;
+};
+
+} // namespace mf

@@ -1,0 +1,210 @@
+"""GPU parity tests: the CUDA path, called through the C ABI, against the CPU oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star, A17): max relative difference <= 1e-11 per field after 100 steps.
+The strict build (no FMA contraction, same operation order) must match the oracle to the last bit where no
+transcendental is involved, which separates "rounding" from "bug".
+"""
+import numpy as np
+import pytest
+
+import parity
+from paper_1510_06340_b200 import workloads as w
+from paper_1510_06340_b200.binding import MustaForce, MustaForceError, MF_ESTATE
+
+pytestmark = pytest.mark.gpu
+
+PATHS = ["staged", "fused"]
+
+
+def _skip_unsupported(fn):
+    try:
+        return fn()
+    except MustaForceError as e:
+        if "fused path does not support" in str(e):
+            pytest.skip("fused path does not support this configuration")
+        raise
+
+
+# ------------------------------------------------------------------ the five configs, 100 steps, scaled grids
+def _scaled(index):
+    if index == 1:
+        return w.shock_tube_1d()                                             # full size: 400 cells
+    if index == 2:
+        return w.diagonal_shock_3d(shape=(40, 36, 44))
+    if index == 3:
+        return w.gaussian_hot_spot(shape=(40, 36, 44), dx=0.2)
+    if index == 4:
+        return w.lumpy_event(shape=(36, 44, 40), dx=0.3)
+    st = w.jet_event(shape=(36, 40, 44), dx=0.3)
+    st["jet"] = dict(dEdx=5.0, sigma=0.6, x0=-4.0, y0=0.0, z0=0.0)           # sigma/dx = 2 on the coarse grid
+    return st
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("index", [1, 2, 3, 4, 5])
+def test_config_100_steps(index, path):
+    st = _scaled(index)
+    g, o = _skip_unsupported(lambda: parity.make_pair(st, path=path))
+    g.step(100, st["cfl"])
+    o.step(100, st["cfl"])
+    got, ref = g.get_state(), o.get_state()
+    assert g.last_status == 0 and o.status() == 0
+    r = parity.assert_parity(got, ref, what="config %d (%s)" % (index, path))
+    tg, to = g.time(), o.time()
+    assert tg[2] == to[2] == 100
+    assert tg[0] == pytest.approx(to[0], rel=1e-12)
+    print("config", index, path, "rel diff E,M,R =", r)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config1_to_t12_matches_oracle_and_exact_solution(path):
+    import exact_riemann
+    st = w.shock_tube_1d()
+    g, o = _skip_unsupported(lambda: parity.make_pair(st, path=path))
+    for h in (g, o):
+        while True:
+            t = h.time()[0]
+            if t >= 12.0 - 1e-12:
+                break
+            smax, _ = h.max_signal_speed()
+            dt = 0.4 * st["dx"] / smax
+            if t + dt > 12.0:
+                h.step_dt(1, 12.0 - t)
+            else:
+                h.step(1, 0.4)
+    parity.assert_parity(g.get_state(), o.get_state(), what="config 1 to t=12")
+    e, vx, _, _, n = [a.ravel() for a in g.get_state_prim()]
+    x = w.centres(400, st["dx"])
+    ee, ve, ne = exact_riemann.exact(x / 12.0, 10.0, 1.0, 10.0, 1.0)
+    assert st["dx"] * np.abs(e - ee).sum() <= 2.0
+    assert st["dx"] * np.abs(vx - ve).sum() <= 0.25
+    assert st["dx"] * np.abs(n - ne).sum() <= 2.4
+
+
+# ------------------------------------------------------------------ strict build: bit-for-bit
+CASES = [("minmod", 2, 2, "outflow", True), ("superbee", 3, 3, "periodic", True), ("mc", 2, 2, "outflow", True),
+         ("vanleer", 1, 3, "periodic", False), ("vanalbada", 4, 3, "outflow", True), ("none", 0, 2, "periodic", True),
+         ("first", 2, 3, "outflow", False)]
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("limiter,k,rk,bc,predictor", CASES)
+@pytest.mark.parametrize("shape", [(1, 1, 37), (9, 11, 13), (1, 12, 10), (7, 1, 9)])
+def test_strict_build_is_bit_identical(shape, limiter, k, rk, bc, predictor, path):
+    rng = np.random.default_rng(5)
+    st = w.lumpy_event(shape=shape, dx=0.25, n_gauss=6, radius=1.0, half_z=0.8, background=0.5)
+    e = st["E"]
+    v = [0.4 * np.sin(1.3 * e), 0.3 * np.cos(0.9 * e) - 0.1, 0.2 * np.sin(0.5 * e + 2)]
+    for d in range(3):
+        if shape[2 - d] == 1:
+            v[d] = 0.0 * e
+    n = 1.0 + rng.uniform(size=shape)
+    over = dict(limiter=limiter, k_stages=k, rk=rk, bc=bc, predictor=predictor)
+    g, o = _skip_unsupported(lambda: parity.make_pair(st, path=path, strict=True, **over))
+    g.set_state_prim(e, v[0], v[1], v[2], n)
+    o.set_state_prim(e, v[0], v[1], v[2], n)
+    for a, b in zip(g.get_state(), o.get_state()):                   # Eq.4 on the device, same order
+        assert np.array_equal(a, b)
+    sg, so = g.max_signal_speed()[0], o.max_signal_speed()[0]
+    assert sg == so
+    g.step(7, 0.3)
+    o.step(7, 0.3)
+    g.step_dt(2, 0.01)
+    o.step_dt(2, 0.01)
+    for q, (a, b) in enumerate(zip(g.get_state(), o.get_state())):
+        assert np.array_equal(a, b), "field %d differs: max abs %g" % (q, np.abs(a - b).max())
+    assert g.time() == o.time()
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_strict_eval_L_and_guarded_states(path):
+    """Near-vacuum and superluminal cells take the A12 guard identically."""
+    rng = np.random.default_rng(6)
+    shape = (6, 7, 9)
+    U = np.zeros((5,) + shape)
+    U[0] = 10 ** rng.uniform(-14, 0, size=shape)
+    for q in (1, 2, 3):
+        U[q] = U[0] * rng.uniform(-0.7, 0.7, size=shape)
+    U[4] = 1.0
+    st = dict(shape=shape, dx=0.1, scheme=dict(limiter="minmod", k_stages=2, rk=2, bc="outflow"),
+              E=U[0], Mx=U[1], My=U[2], Mz=U[3], R=U[4])
+    g, o = _skip_unsupported(lambda: parity.make_pair(st, path=path, strict=True))
+    for a, b in zip(g.eval_L(0.02), o.eval_L(0.02)):
+        assert np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------ invariants on the GPU itself
+@pytest.mark.parametrize("path", PATHS)
+def test_gpu_conservation_and_uniform_state(path):
+    st = w.gaussian_hot_spot(shape=(48, 40, 56), dx=0.15)
+    g = _skip_unsupported(lambda: MustaForce(56, 40, 48, dx=0.15, limiter="superbee", k_stages=3, rk=3, bc="periodic", path=path))
+    g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+    t0 = g.totals()
+    g.step(50, 0.3)
+    t1 = g.totals()
+    assert abs(t1[0] - t0[0]) / t0[0] <= 1e-12
+    assert abs(t1[4] - t0[4]) / t0[4] <= 1e-12
+    assert max(abs(t1[q]) for q in (1, 2, 3)) / t0[0] <= 1e-12
+    n = 56 * 40 * 48
+    g.set_state_prim(np.full(n, 2.0), np.full(n, 0.3), np.full(n, -0.2), np.full(n, 0.5), np.full(n, 1.5))
+    before = g.get_state()
+    g.step(3, 0.3)
+    for a, b in zip(g.get_state(), before):
+        assert np.allclose(a, b, rtol=3e-15, atol=0)
+
+
+def test_totals_match_oracle():
+    st = w.lumpy_event(shape=(20, 24, 28), dx=0.3)
+    g, o = parity.make_pair(st)
+    assert np.allclose(g.totals(), o.totals(), rtol=1e-14, atol=1e-300)
+
+
+def test_bad_state_raises_sticky_estate():
+    st = w.shock_tube_1d(nx=64, length=6.4)
+    g = MustaForce(64, dx=0.1)
+    E = st["E"].copy()
+    E.ravel()[10] = np.nan
+    g.set_state(E, st["Mx"], st["My"], st["Mz"], st["R"])
+    g.step(1, 0.4)
+    assert g.sync() == MF_ESTATE
+    g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])      # reset clears it
+    g.step(1, 0.4)
+    assert g.sync() == 0
+    Mx = st["Mx"].copy()
+    Mx.ravel()[5] = 50.0                                             # |M| > E
+    g.set_state(st["E"], Mx, st["My"], st["Mz"], st["R"])
+    assert g.max_signal_speed()[1] == MF_ESTATE
+
+
+def test_empty_and_argument_errors():
+    g = MustaForce(16, dx=0.1)
+    g.step(0, 0.4)                                                    # zero steps is a no-op
+    assert g.time()[2] == 0
+    with pytest.raises(MustaForceError):
+        g.step(1, -1.0)
+    with pytest.raises(MustaForceError):
+        MustaForce(3, dx=0.1)                                         # active axis needs >= 4
+    with pytest.raises(MustaForceError):
+        MustaForce(16, dx=0.1, k_stages=9)
+    with pytest.raises(ValueError):
+        g.set_state(np.zeros(3), np.zeros(3), np.zeros(3), np.zeros(3), np.zeros(3))
+
+
+def test_device_pointer_state_io_and_user_stream():
+    import torch
+    st = w.lumpy_event(shape=(12, 14, 16), dx=0.3)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        g = MustaForce(16, 14, 12, dx=0.3, stream=s.cuda_stream)
+        dev = [torch.from_numpy(np.ascontiguousarray(st[k])).cuda() for k in ("E", "Mx", "My", "Mz", "R")]
+        s.synchronize()
+        g.set_state_device([t.data_ptr() for t in dev])
+        g.step(5, 0.3)
+        out = [torch.empty_like(t) for t in dev]
+        g.get_state_device([t.data_ptr() for t in out])
+    h = MustaForce(16, 14, 12, dx=0.3)
+    h.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+    h.step(5, 0.3)
+    for a, b in zip(out, h.get_state()):
+        assert np.array_equal(a.cpu().numpy().reshape(b.shape), b)
+    assert g.launch_count() > 0
