@@ -33,10 +33,11 @@ def _scaled(index):
         return w.diagonal_shock_3d(shape=(40, 36, 44))
     if index == 3:
         return w.gaussian_hot_spot(shape=(40, 36, 44), dx=0.2)
-    if index == 4:
-        return w.lumpy_event(shape=(36, 44, 40), dx=0.3)
-    st = w.jet_event(shape=(36, 40, 44), dx=0.3)
-    st["jet"] = dict(dEdx=5.0, sigma=0.6, x0=-4.0, y0=0.0, z0=0.0)           # sigma/dx = 2 on the coarse grid
+    if index == 4:                                                           # same dx and Gaussian width as config 4, fewer
+        return w.lumpy_event(shape=(36, 44, 40), dx=0.1, n_gauss=10, radius=1.2, half_z=0.8)    # hot spots in a smaller box
+    st = w.lumpy_event(event=1000, shape=(36, 40, 44), dx=0.1, n_gauss=10, radius=1.2, half_z=0.8)
+    st.update(scheme=dict(limiter="mc", k_stages=3, rk=3, bc="outflow"), cfl=0.3,
+              jet=dict(dEdx=5.0, sigma=0.3, x0=-1.5, y0=0.0, z0=0.0))
     return st
 
 
