@@ -1,0 +1,339 @@
+#!/usr/bin/env python
+"""bench.py — fp64 cell-updates/s of the MUSTA-FORCE step (BASELINE.json metric) on N GPUs of one node.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--grid nz,ny,nx] [--path auto]
+
+A "step" is one pass of the whole hot path (CFL reduction, all RK stages: ghost handling, limited reconstruction,
+Hancock predictor, MUSTA/FORCE fluxes with con2prim, flux divergence, RK combine) over one synthetic grid.
+Default workload: BASELINE.json config 3 (the one the metric is quoted on): 256^3 periodic Gaussian hot spot,
+dx 0.05, k=3, superbee, RK3, cfl 0.3.  N > 1 runs N independent replicas (the path does not shard in this build,
+DESIGN.md "Multi-GPU"): weak scaling, no data-path collective.
+
+One JSON line on stdout (rank 0).  --impl reference times the CPU oracle (oracle/) on a bounded sample instead.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1510_06340_b200 import workloads  # noqa: E402
+from paper_1510_06340_b200.replicas import Replicas  # noqa: E402
+
+METRIC = "fp64 cell-updates/s, MUSTA-FORCE step"
+UNIT = "cell-updates/s"
+
+# ----------------------------------------------------------------------------------------------------------------
+# Algorithmic work per cell-update.  FP64-pipe issue SLOTS:
+# add/sub/mul/fma/compare/min/max = 1, divide = 8, square root = 8 (a Newton sequence each); abs/neg/select = 0.
+DIV, SQRT = 8, 8
+FLUX = 16 + DIV + SQRT                    # a6: one flux evaluation with con2prim             = 32
+SLOPE = {"none": 2, "first": 0, "minmod": 3, "superbee": 7, "mc": 8, "vanleer": 4 + DIV, "vanalbada": 6 + DIV}
+
+
+def alg_slots(limiter, k, rk, ndim, predictor=True):
+    """(slots per cell-update, slots per L-evaluation, slots of the MUSTA fluxes per L-evaluation)."""
+    recon = 5 * ndim * (4 + SLOPE[limiter])                        # a3: a, b, slope, two face values
+    pred = (2 * ndim * FLUX + 5 * 4 * ndim) if predictor else 0     # a4: 2D flux evaluations + delta + 2D face updates
+    force = 3 * FLUX + 50                                           # Eq.9-11: three fluxes + 10 per component
+    musta = (k + 1) * force + 20 * k                                # a5: k Eq.8 updates
+    comb = 5 * (2 * ndim + 5)                                       # a7: divergence + RK form
+    cfl = (16 + DIV + SQRT) + (3 + SQRT) + (2 + DIV) + 1            # a2
+    per_L = recon + pred + ndim * musta + comb
+    return rk * per_L + cfl, per_L, ndim * musta
+
+
+def alg_bytes(rk):
+    """Minimum HBM bytes per cell-update: stage 1 reads U^n writes U1 (80 B), later stages read U_s and U^n, write (120 B); CFL +32 B."""
+    return 80 + 120 * (rk - 1) + 32
+
+
+FP64_LANES_PER_SM = 64        # B200 (sm_100): 4 SMSPs x 16 FP64 lanes; mf_probe_fp64 measures it
+
+
+def peaks():
+    mp = {}
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        mp = json.load(open(path))
+    hbm = mp.get("hbm_gbs", 6650.0)
+    return dict(hbm_gbs=hbm, hbm_source="measured (MEASURED_PEAKS.json)" if "hbm_gbs" in mp else "fallback (B200_PROFILING.md)",
+                sm_max_mhz=mp.get("sm_max_mhz", 1965.0))
+
+
+# ----------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi samples of SM clock and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index=0):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "--id=%d" % self.index, "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0=None, t1=None):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        clocks, maxc, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.lines:
+            if t0 is not None and not (t0 <= ts <= t1 + 0.1):
+                continue
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                clocks.append(float(f[0])); maxc.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nme, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nme)
+        if not clocks:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples in the timed region"], "samples": 0}
+        return {"sm_mhz": float(np.median(clocks)), "sm_max_mhz": float(max(maxc)), "reasons": sorted(reasons),
+                "samples": len(clocks), "power_w_max": max(power)}
+
+
+def make_workload(args):
+    shape = tuple(int(x) for x in args.grid.split(",")) if args.grid else None
+    if args.config == 3 and shape is None:
+        return workloads.gaussian_hot_spot()
+    return workloads.config(args.config, scale=shape)
+
+
+def describe(st, extra=None):
+    nz, ny, nx = st["shape"]
+    cfg = {"workload": "%s %dx%dx%d dx=%g %s k=%d RK%d %s cfl=%g" % (
+        st["name"], nx, ny, nz, st["dx"], st["scheme"]["limiter"], st["scheme"]["k_stages"], st["scheme"]["rk"],
+        st["scheme"]["bc"], st["cfl"]), "cells": nx * ny * nz, "predictor": "on (paper-literal Eq.13)"}
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def centre_crop(st, m):
+    """A centred m^3 (or smaller) sub-box of the workload: the bounded sample the CPU oracle is timed on."""
+    nz, ny, nx = st["shape"]
+    cz, cy, cx = min(m, nz), min(m, ny), min(m, nx)
+    z0, y0, x0 = (nz - cz) // 2, (ny - cy) // 2, (nx - cx) // 2
+    out = dict(st)
+    for key in ("E", "Mx", "My", "Mz", "R"):
+        out[key] = np.ascontiguousarray(st[key][z0:z0 + cz, y0:y0 + cy, x0:x0 + cx])
+    out["shape"] = (cz, cy, cx)
+    return out
+
+
+class OracleSample:
+    """The CPU oracle as it stands (oracle/libmfo.so, one thread, never tuned for this) on a centred crop."""
+
+    def __init__(self, st, crop):
+        from oracle.mfo import Oracle, num_threads
+        self.st = centre_crop(st, crop)
+        nz, ny, nx = self.st["shape"]
+        self.cells = nx * ny * nz
+        self.o = Oracle(nx, ny, nz, dx=st["dx"], omp=False, **st["scheme"])
+        self.o.set_state(self.st["E"], self.st["Mx"], self.st["My"], self.st["Mz"], self.st["R"])
+        if "jet" in st:
+            j = st["jet"]
+            self.o.set_jet_source(j["dEdx"], j["sigma"], j["x0"], j["y0"], j["z0"])
+        self.cores = num_threads(False)
+        self.cfl = st["cfl"]
+        self.sample = "centred %dx%dx%d crop of the workload's initial state, same scheme" % (nx, ny, nz)
+
+    def time_steps(self, steps):
+        t0 = time.perf_counter()
+        self.o.step(steps, self.cfl)
+        return time.perf_counter() - t0
+
+
+def cpu_baseline(st, budget_s=12.0, crop=64):
+    s = OracleSample(st, crop)
+    one = s.time_steps(1)                                     # also the warm-up
+    n = max(1, min(50, int(budget_s / max(one, 1e-6))))
+    dt = s.time_steps(n)
+    return {"value": s.cells * n / dt, "unit": UNIT, "cores": s.cores, "kind": "oracle",
+            "sample": "%s, %d steps in %.1f s" % (s.sample, n, dt)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the box's host cores, K timed steps after W warm-up steps of a bounded sample."""
+    rep = Replicas(backend="gloo")
+    if rep.rank != 0:
+        return
+    st = make_workload(args)
+    s = OracleSample(st, args.ref_crop)
+    s.time_steps(max(args.warmup, 1))
+    dt = s.time_steps(args.steps)
+    value = s.cells * args.steps / dt
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": describe(st, {"sample": s.sample}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": s.cores, "kind": "oracle", "sample": s.sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_1510_06340_b200 import binding
+    from paper_1510_06340_b200.binding import MustaForce
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback (use --impl reference for the oracle)")
+    rank, local_rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    torch.cuda.set_device(local_rank)
+    rep = Replicas(backend="nccl", device=torch.device("cuda", local_rank))
+    st = make_workload(args)
+    nz, ny, nx = st["shape"]
+    cells = nx * ny * nz
+    sch = st["scheme"]
+    ndim = sum(1 for n in (nx, ny, nz) if n > 1)
+
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        g = MustaForce(nx, ny, nz, dx=st["dx"], path=args.path, stream=stream.cuda_stream, **sch)
+        if "jet" in st:
+            j = st["jet"]
+            g.set_jet_source(j["dEdx"], j["sigma"], j["x0"], j["y0"], j["z0"])
+        fields = ("E", "Mx", "My", "Mz", "R")
+        # device-resident inputs for the kernel-throughput leg
+        dev = [torch.from_numpy(np.ascontiguousarray(st[f])).to("cuda", non_blocking=False) for f in fields]
+        stream.synchronize()
+        g.set_state_device([t.data_ptr() for t in dev])
+        g.step(args.warmup, st["cfl"])
+        g.sync()
+        rep.barrier()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        l0 = g.launch_count()
+        g.profile(True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(stream)
+        g.step(args.steps, st["cfl"])
+        e1.record(stream)
+        stream.synchronize()
+        rep.barrier()
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        clocks = sampler.stop(t0, t1)
+        g.profile(False)
+        prof = g.profile_read()
+        launches = g.launch_count() - l0
+        elapsed_ms = rep.max(e0.elapsed_time(e1))
+        status = g.sync()
+        value = rep.sum(cells * args.steps) / (elapsed_ms * 1e-3)
+
+        # ---- end to end through the C ABI with HOST buffers: H2D of the step's input and D2H of its result inside the timed region
+        pin_in = [torch.from_numpy(np.ascontiguousarray(st[f])).pin_memory() for f in fields]
+        pin_out = [torch.empty_like(t).pin_memory() for t in pin_in]
+        np_in = [t.numpy() for t in pin_in]
+        np_out = [t.numpy() for t in pin_out]
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        for _ in range(2):
+            g.set_state(*np_in); g.step(1, st["cfl"]); g.get_state(out=np_out)
+        rep.barrier()
+        torch.cuda.synchronize()
+        w0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            g.set_state(*np_in)
+            g.step(1, st["cfl"])
+            g.get_state(out=np_out)
+        torch.cuda.synchronize()
+        e2e_s = rep.max(time.perf_counter() - w0)
+        e2e_value = rep.sum(cells * e2e_steps) / e2e_s
+
+    if rank != 0:
+        rep.close()
+        return
+
+    pk = peaks()
+    slots_cu, slots_L, slots_musta = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim)
+    alu_peak_slots = 148 * FP64_LANES_PER_SM * pk["sm_max_mhz"] * 1e6          # FP64 instructions/s, all SMs
+    # dominant kernel, from the event pairs recorded around every launch inside the timed region
+    dom = max((k for k in prof if k in ("fused_stage", "flux_stage")), key=lambda k: prof[k][0], default=None)
+    roof = None
+    if dom:
+        ms, groups = prof[dom]
+        per_launch_slots = (slots_L if dom == "fused_stage" else slots_musta) * cells
+        achieved = 2.0 * per_launch_slots / (ms / groups * 1e-3) / 1e12
+        peak = 2.0 * alu_peak_slots / 1e12
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                "kernel": dom, "launch_ms": ms / groups, "share_of_step": ms / elapsed_ms,
+                "note": "FMA-equivalent flops = 2 x algorithmic FP64 issue slots (div = sqrt = 8 slots); peak = 2 x 148 SM x 64 lanes x clocks.max.sm"}
+    step_frac_alu = (slots_cu * cells * args.steps / (elapsed_ms * 1e-3)) / alu_peak_slots
+    step_frac_hbm = (alg_bytes(sch["rk"]) * cells * args.steps / (elapsed_ms * 1e-3)) / (pk["hbm_gbs"] * 1e9)
+    probe = binding.probe_fp64()
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": describe(st, {"path": g.path(), "l2": "state registers (%.0f MB each) exceed the 126 MB L2" % (40e-6 * cells)
+                                    if 40 * cells > 126e6 else "state fits in L2 (small grid)", "parallelism": "replicas x%d" % world,
+                                    "status": status}),
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 40 * cells, "d2h_bytes_per_step": 40 * cells,
+                    "steps": e2e_steps, "note": "mf_set_state(host) + mf_step(1) + mf_get_state(host) per step, pinned host buffers"},
+            "gpu_launches": launches,
+            "roofline": roof,
+            "roofline_step": {"alg_slots_per_cell_update": slots_cu, "alg_bytes_per_cell_update": alg_bytes(sch["rk"]),
+                              "frac_alu": step_frac_alu, "frac_hbm": step_frac_hbm, "hbm_peak": pk["hbm_source"],
+                              "measured_dfma_per_s": probe["dfma_per_s"], "measured_rcp_slots": probe["dfma_per_s"] / probe["rcp_per_s"],
+                              "measured_sqrt_slots": probe["dfma_per_s"] / probe["sqrt_per_s"]},
+            "kernels_ms": {k: {"ms_total": v[0], "groups": v[1]} for k, v in prof.items()}}
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(st, crop=args.ref_crop)
+    print(json.dumps(line), flush=True)
+    rep.close()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (default 3 = the 256^3 metric workload)")
+    ap.add_argument("--grid", default=None, help="nz,ny,nx override (parity/debug sizes)")
+    ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--ref-crop", type=int, default=64, help="edge of the centred crop the CPU oracle is timed on")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -180,7 +180,7 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
 // =========================================================================== a5 + a6: interface fluxes
 // One thread per interface between cell c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
 template <int D>
-__global__ void __launch_bounds__(TPB) k_flux_stage(Grid g, Eos q, int k, Faces fc, Fluxes fx, const StepState* ds)
+__global__ void __launch_bounds__(TPB, 3) k_flux_stage(Grid g, Eos q, int k, Faces fc, Fluxes fx, const StepState* ds)
 {
     int m[3] = { g.n[0], g.n[1], g.n[2] };
     m[D] += 1;
