@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -31,6 +32,8 @@ struct mf_ctx {
     int cur;                 // which register holds U^n
     double* faces;           // staged path: 2*5*nact*next doubles
     double* fluxes;          // staged path: 5*nact*next doubles
+    double* delta;           // fused path: Hancock increment, 5*next doubles
+    int sweep_variant;       // fused path tile shape (tuning knob, env MF_SWEEP_VARIANT at mf_create)
     StepState* ds;
     StepState* h_ds;         // pinned mirror
     double* partials;        // totals: 5*nblocks doubles
@@ -90,13 +93,16 @@ void set_eos(Eos& q, double cs2)
     q.c1sq = q.c1 * q.c1;
     q.four_cs2 = 4.0 * cs2;
     q.cs = std::sqrt(cs2);
+    q.qc1sq = 0.25 * q.c1sq;
+    q.hc1 = 0.5 * q.c1;
+    q.vcap2 = V_CAP * V_CAP;
 }
 
 int resolve_path(mf_ctx* c)
 {
     if (c->path_req == MF_PATH_FUSED) { if (!fused_supported(c->g)) return MF_EINVAL; c->path = MF_PATH_FUSED; }
     else if (c->path_req == MF_PATH_STAGED) c->path = MF_PATH_STAGED;
-    else c->path = fused_supported(c->g) ? MF_PATH_FUSED : MF_PATH_STAGED;
+    else c->path = MF_PATH_STAGED;      // measured faster than the fused path on B200 so far (profiles/)
     return MF_OK;
 }
 
@@ -137,9 +143,18 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
 {
     const long long n = c->g.ncell;
     if (c->path == MF_PATH_FUSED) {
-        int ps = prof_begin(c, 4);
-        c->launches += launch_fused_stage(c->g, c->q, c->limiter, c->predictor, c->k, cstate(V, n), sg, cstate(Ua, n), cstate(V, n),
-                                          state(out, n), c->src, c->ds, c->num_sms, c->stream);
+        if (!c->delta) {
+            if (cudaMalloc(&c->delta, sizeof(double) * 5 * c->g.next) != cudaSuccess) { cudaGetLastError(); c->delta = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(delta) failed"); }
+        }
+        int ps;
+        if (c->predictor) {
+            ps = prof_begin(c, 1);
+            c->launches += launch_delta_stage(c->g, c->q, c->limiter, cstate(V, n), state(c->delta, c->g.next), c->ds, c->stream);
+            prof_end(c, ps);
+        }
+        ps = prof_begin(c, 4);
+        c->launches += launch_fused_stage(c->g, c->q, c->limiter, c->predictor, c->k, cstate(V, n), cstate(c->delta, c->g.next), sg, cstate(Ua, n),
+                                          state(out, n), c->src, c->ds, c->num_sms, c->sweep_variant, c->stream);
         prof_end(c, ps);
     } else {
         int rc = ensure_staged_buffers(c);
@@ -150,7 +165,7 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
         c->launches += launch_cell_stage(c->g, c->q, c->limiter, c->predictor, cstate(V, n), fc, c->ds, c->stream);
         prof_end(c, ps);
         ps = prof_begin(c, 2);
-        c->launches += launch_flux_stage(c->g, c->q, c->k, fc, fx, c->ds, c->stream);
+        c->launches += launch_flux_stage(c->g, c->q, c->k, 7, fc, fx, c->ds, c->stream);
         prof_end(c, ps);
         ps = prof_begin(c, 3);
         c->launches += launch_combine(c->g, fx, sg, cstate(Ua, n), cstate(V, n), state(out, n), c->src, c->ds, c->stream);
@@ -227,7 +242,8 @@ mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k
     mf_ctx* c = new (std::nothrow) mf_ctx();
     if (!c) { fail(nullptr, MF_ENOMEM, "host allocation failed"); return nullptr; }
     memset(&c->g, 0, sizeof(c->g));
-    c->U[0] = c->U[1] = c->U[2] = nullptr; c->faces = c->fluxes = nullptr; c->ds = nullptr; c->h_ds = nullptr;
+    c->U[0] = c->U[1] = c->U[2] = nullptr; c->faces = c->fluxes = nullptr; c->delta = nullptr;
+    { const char* v = getenv("MF_SWEEP_VARIANT"); c->sweep_variant = v ? atoi(v) : 0; } c->ds = nullptr; c->h_ds = nullptr;
     c->partials = nullptr; c->h_partials = nullptr; c->own_stream = nullptr; c->stream = nullptr;
     cudaGetDevice(&c->dev);
     cudaDeviceProp prop;
@@ -286,6 +302,7 @@ void mf_destroy(mf_ctx* c)
     for (int r = 0; r < 3; ++r) if (c->U[r]) cudaFree(c->U[r]);
     if (c->faces) cudaFree(c->faces);
     if (c->fluxes) cudaFree(c->fluxes);
+    if (c->delta) cudaFree(c->delta);
     if (c->ds) cudaFree(c->ds);
     if (c->h_ds) cudaFreeHost(c->h_ds);
     if (c->partials) cudaFree(c->partials);

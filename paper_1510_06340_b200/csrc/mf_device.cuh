@@ -18,6 +18,10 @@ struct Eos {
     double c1sq;    // c1*c1
     double four_cs2;
     double cs;      // sqrt(cs2)
+    // derived constants of the product build's fast flux (not used by the strict build)
+    double qc1sq;   // c1*c1/4
+    double hc1;     // c1/2
+    double vcap2;   // V_CAP^2
 };
 
 // ---- Eq.14-21 in two-argument form (A6): a = U_i - U_{i-1}, b = U_{i+1} - U_i; returns the limited slope
@@ -115,12 +119,57 @@ __device__ __forceinline__ void flux_d(const Eos& q, const double (&U)[5], doubl
     F[4] = U[4] * vd;
 }
 
+#ifndef MF_STRICT
+// Product build: the same flux on the admissible fast path with the minimum number of FP64-pipe instructions (26):
+//   Q/2 = sqrt(c1^2/4 E^2 - cs2 |M|^2),  inv = 1/(c1/2 E + Q/2) = 2/(c1 E + Q),  v_d = M_d inv,  p = cs2 (E - |M|^2 inv),
+//   F_E = M_d  (reading A15: (E+p) v_d == M_d identically when the guard is inactive).
+// Returns false when the state needs the guarded general path (vacuum, NaN, |M| > V_CAP E); the caller then calls flux_d.
+// The vacuum test compares the high word of E as an integer (conservative: borderline values take the general path).
+template <int D>
+__device__ __forceinline__ bool flux_fast(const Eos& q, const double (&U)[5], double (&F)[5])
+{
+    const double E = U[0];
+    const double M2 = fma(U[3], U[3], fma(U[2], U[2], U[1] * U[1]));
+    const double EE = E * E;
+    const bool ok = (__double2hiint(E) > 0x3D719799) && (M2 <= q.vcap2 * EE);
+    const double Qh = sqrt_pos(fma(-q.cs2, M2, q.qc1sq * EE));
+    double y;
+    {
+        const double x = fma(q.hc1, E, Qh);
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+        const double e1 = fma(-x, y, 1.0);
+        y = fma(y, fma(e1, e1, e1), y);
+    }
+    const double vd = U[1 + D] * y;
+    const double p = q.cs2 * fma(-M2, y, E);
+    F[0] = U[1 + D];
+    F[1] = U[1] * vd;
+    F[2] = U[2] * vd;
+    F[3] = U[3] * vd;
+    F[1 + D] += p;
+    F[4] = U[4] * vd;
+    return ok;
+}
+#endif
+
+// flux evaluation used outside MUSTA (Hancock predictor): fast path with the guarded fallback
+template <int D>
+__device__ __forceinline__ void flux_eval(const Eos& q, const double (&U)[5], double (&F)[5])
+{
+#ifdef MF_STRICT
+    flux_d<D>(q, U, F);
+#else
+    if (!flux_fast<D>(q, U, F)) flux_d<D>(q, U, F);
+#endif
+}
+
 // ---- MUSTA_k with FORCE-alpha, steps 1-5 :123-135, Eq.8-11 :130-149 (A1: Richtmyer state uses the flux difference)
 // A, B are U_L^(0), U_R^(0) on entry and are overwritten.
 template <int D>
 __device__ __forceinline__ void musta_flux(const Eos& q, int k, double lam, double c_lw, double c_lf,
                                            double (&A)[5], double (&B)[5], double (&F)[5])
 {
+#ifdef MF_STRICT
     for (int l = 0;; ++l) {
         double FA[5], FB[5], W[5];
         flux_d<D>(q, A, FA);
@@ -140,6 +189,28 @@ __device__ __forceinline__ void musta_flux(const Eos& q, int k, double lam, doub
             B[c] = B[c] - lam * (FB[c] - F[c]);
         }
     }
+#else
+    // same formulas with the constant factors folded so that every line is one FP64 instruction
+    const double hc_lf = 0.5 * c_lf;
+    for (int l = 0;; ++l) {
+        double FA[5], FB[5], W[5];
+        const bool okA = flux_fast<D>(q, A, FA);
+        const bool okB = flux_fast<D>(q, B, FB);
+        if (!(okA && okB)) { flux_d<D>(q, A, FA); flux_d<D>(q, B, FB); }                     // rare: guarded general path
+#pragma unroll
+        for (int c = 0; c < 5; ++c) W[c] = fma(0.5, A[c] + B[c], -(c_lw * (FB[c] - FA[c])));  // Eq.10
+        if (!flux_fast<D>(q, W, F)) flux_d<D>(q, W, F);                                       // F^lw
+#pragma unroll
+        for (int c = 0; c < 5; ++c)                                                           // Eq.9 with Eq.11 inside
+            F[c] = fma(-hc_lf, B[c] - A[c], fma(0.25, FA[c] + FB[c], 0.5 * F[c]));
+        if (l == k) break;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {                                                         // Eq.8
+            A[c] = fma(-lam, F[c] - FA[c], A[c]);
+            B[c] = fma(-lam, FB[c] - F[c], B[c]);
+        }
+    }
+#endif
 }
 
 // ---- a2: local signal speed (|v|+cs)/(1+|v|cs) (A10) and the state check behind MF_ESTATE
@@ -153,6 +224,8 @@ __device__ __forceinline__ double signal_speed(const Eos& q, double E, double Mx
     double av = sqrt(vx * vx + vy * vy + vz * vz);
     return (av + q.cs) / (1.0 + av * q.cs);
 }
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
 __device__ __forceinline__ int bc_index(int i, int n, int periodic)
 {

@@ -134,19 +134,19 @@ __global__ void __launch_bounds__(TPB) k_cell_stage(Grid g, Eos q, int predictor
         bool first = true;
         double Fl[5], Fr[5];
         if (g.act[0]) {
-            flux_d<0>(q, UL[0], Fl); flux_d<0>(q, UR[0], Fr);
+            flux_eval<0>(q, UL[0], Fl); flux_eval<0>(q, UR[0], Fr);
 #pragma unroll
             for (int v = 0; v < 5; ++v) delta[v] = hl * (Fl[v] - Fr[v]);
             first = false;
         }
         if (g.act[1]) {
-            flux_d<1>(q, UL[1], Fl); flux_d<1>(q, UR[1], Fr);
+            flux_eval<1>(q, UL[1], Fl); flux_eval<1>(q, UR[1], Fr);
 #pragma unroll
             for (int v = 0; v < 5; ++v) { double t = hl * (Fl[v] - Fr[v]); delta[v] = first ? t : delta[v] + t; }
             first = false;
         }
         if (g.act[2]) {
-            flux_d<2>(q, UL[2], Fl); flux_d<2>(q, UR[2], Fr);
+            flux_eval<2>(q, UL[2], Fl); flux_eval<2>(q, UR[2], Fr);
 #pragma unroll
             for (int v = 0; v < 5; ++v) { double t = hl * (Fl[v] - Fr[v]); delta[v] = first ? t : delta[v] + t; }
         }
@@ -202,11 +202,11 @@ __global__ void __launch_bounds__(TPB, 3) k_flux_stage(Grid g, Eos q, int k, Fac
     for (int v = 0; v < 5; ++v) fx.f[D][v][p] = F[v];
 }
 
-int launch_flux_stage(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx, const StepState* ds, cudaStream_t st)
+int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, Fluxes fx, const StepState* ds, cudaStream_t st)
 {
     int launches = 0;
     for (int d = 0; d < 3; ++d) {
-        if (!g.act[d]) continue;
+        if (!g.act[d] || !(dmask & (1 << d))) continue;
         long long total = 1;
         for (int a = 0; a < 3; ++a) total *= (a == d) ? g.n[a] + 1 : g.n[a];
         unsigned int nb = blocks_for(total, TPB);

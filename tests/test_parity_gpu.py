@@ -209,3 +209,69 @@ def test_device_pointer_state_io_and_user_stream():
     for a, b in zip(out, h.get_state()):
         assert np.array_equal(a.cpu().numpy().reshape(b.shape), b)
     assert g.launch_count() > 0
+
+
+# ------------------------------------------------------------------ full-size grids: windowed parity
+def _windowed_parity(st, centre, steps_before=3, m=2, half=8, path="auto"):
+    """Advance the FULL grid on the GPU, then re-run the last m steps with the oracle on a sub-box around `centre`
+    (interior (2*half)^3 plus a halo of 2 cells per RK stage per step), with the GPU's own dt sequence, and compare."""
+    nz, ny, nx = st["shape"]
+    sch = st["scheme"]
+    halo = 2 * sch["rk"] * m
+    g = MustaForce(nx, ny, nz, dx=st["dx"], path=path, **sch)
+    g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+    if "jet" in st:
+        j = st["jet"]
+        g.set_jet_source(j["dEdx"], j["sigma"], j["x0"], j["y0"], j["z0"])
+    g.step(steps_before, st["cfl"])
+    before = g.get_state()
+    t_before = g.time()[0]
+    dts = []
+    for _ in range(m):
+        g.step(1, st["cfl"])
+        dts.append(g.time()[1])
+    after = g.get_state()
+    assert g.last_status == 0
+    lo = [c - half - halo for c in centre]
+    hi = [c + half + halo for c in centre]
+    assert min(lo) >= 0 and hi[0] <= nz and hi[1] <= ny and hi[2] <= nx
+    sl = tuple(slice(a, b) for a, b in zip(lo, hi))
+    w = hi[0] - lo[0]
+    from oracle.mfo import Oracle
+    o = Oracle(w, w, w, dx=st["dx"], omp=True, **dict(sch, bc="outflow"))
+    o.set_state(*[np.ascontiguousarray(f[sl]) for f in before])
+    if "jet" in st:
+        # the window's cell centres are shifted by `off` against the full grid's; move the source accordingly
+        j = st["jet"]
+        off = [(lo[a] + w / 2.0 - n / 2.0) * st["dx"] for a, n in zip(range(3), (nz, ny, nx))]
+        o.set_jet_source(j["dEdx"], j["sigma"], j["x0"] + t_before - off[2], j["y0"] - off[1], j["z0"] - off[0])
+    for dt in dts:
+        o.step_dt(1, dt)
+    ref = o.get_state()
+    inner = (slice(halo, w - halo),) * 3
+    got = [f[sl][inner] for f in after]
+    # A17's denominators are the max-norms of the whole field, not of the window
+    return parity.assert_parity(got, [f[inner] for f in ref], what="window at %s" % (centre,), scales=parity.field_scales(after))
+
+
+def test_full_size_config3_256_windows():
+    """BASELINE.json config 3 at full size, in the configuration bench.py times: windows at the hot spot and off centre."""
+    st = w.gaussian_hot_spot()
+    for centre in ((128, 128, 128), (100, 140, 90), (40, 128, 200)):
+        r = _windowed_parity(st, centre)
+        print("256^3 window", centre, r)
+
+
+def test_full_size_config2_128_window():
+    st = w.diagonal_shock_3d()
+    r = _windowed_parity(st, (64, 64, 64), steps_before=10)          # the shock front passes through the centre
+    print("128^3 window", r)
+
+
+def test_full_size_config5_512_window_with_jet():
+    """Largest configuration (512^3, 5 GB per state): a window on the jet source."""
+    st = w.jet_event()
+    nz, ny, nx = st["shape"]
+    jx = int(round((st["jet"]["x0"]) / st["dx"] + nx / 2.0))
+    r = _windowed_parity(st, (nz // 2, ny // 2, jx), steps_before=2, m=1, half=8)
+    print("512^3 window", r)
