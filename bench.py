@@ -321,7 +321,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (default 3 = the 256^3 metric workload)")
     ap.add_argument("--grid", default=None, help="nz,ny,nx override (parity/debug sizes)")
-    ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused"])
+    ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--ref-crop", type=int, default=64, help="edge of the centred crop the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -49,7 +49,8 @@ enum { MF_BC_OUTFLOW = 0 /* clamp index per axis */, MF_BC_PERIODIC = 1 /* index
 enum { MF_OK = 0, MF_EINVAL = -1, MF_ENOMEM = -2, MF_ECUDA = -3, MF_ESTATE = -4 };
 enum { MF_PATH_AUTO = 0   /* fastest path that supports the configuration */,
        MF_PATH_STAGED = 1 /* three kernels per RK stage, face states and fluxes through HBM */,
-       MF_PATH_FUSED = 2  /* one kernel per RK stage, face states and fluxes on chip */ };
+       MF_PATH_FUSED = 2  /* predictor kernel + one tile kernel per RK stage: face states, fluxes and differences on chip (3D grids) */,
+       MF_PATH_HYBRID = 3 /* the staged cell stage + the tile kernel (3D grids) */ };
 
 /* Create a context for an nx*ny*nz grid of spacing dx (same on every axis).  An axis of extent 1 is inactive
  * (ny = nz = 1 is the 1D scheme); an active axis needs extent >= 4.  0 <= k_stages <= 8 is the number of Eq.8

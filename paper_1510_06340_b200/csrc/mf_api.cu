@@ -33,7 +33,7 @@ struct mf_ctx {
     double* faces;           // staged path: 2*5*nact*next doubles
     double* fluxes;          // staged path: 5*nact*next doubles
     double* delta;           // fused path: Hancock increment, 5*next doubles
-    int sweep_variant;       // fused path tile shape (tuning knob, env MF_SWEEP_VARIANT at mf_create)
+    int smax_valid;          // the device-side S_max accumulator already holds the reduction of the current U^n (fused into the last combine)
     StepState* ds;
     StepState* h_ds;         // pinned mirror
     double* partials;        // totals: 5*nblocks doubles
@@ -100,7 +100,7 @@ void set_eos(Eos& q, double cs2)
 
 int resolve_path(mf_ctx* c)
 {
-    if (c->path_req == MF_PATH_FUSED) { if (!fused_supported(c->g)) return MF_EINVAL; c->path = MF_PATH_FUSED; }
+    if (c->path_req == MF_PATH_FUSED || c->path_req == MF_PATH_HYBRID) { if (!fused_supported(c->g)) return MF_EINVAL; c->path = c->path_req; }
     else if (c->path_req == MF_PATH_STAGED) c->path = MF_PATH_STAGED;
     else c->path = MF_PATH_STAGED;      // measured faster than the fused path on B200 so far (profiles/)
     return MF_OK;
@@ -142,7 +142,19 @@ int ensure_staged_buffers(mf_ctx* c)
 int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, double* out)
 {
     const long long n = c->g.ncell;
-    if (c->path == MF_PATH_FUSED) {
+    if (c->path == MF_PATH_FUSED || c->path == MF_PATH_HYBRID) {
+        if (c->path == MF_PATH_HYBRID) {                           // the staged path's cell stage + the tile kernel
+            int rc = ensure_staged_buffers(c);
+            if (rc != MF_OK) return rc;
+            Faces fc = faces_of(c);
+            int ps = prof_begin(c, 1);
+            c->launches += launch_cell_stage(c->g, c->q, c->limiter, c->predictor, cstate(V, n), fc, c->ds, c->stream);
+            prof_end(c, ps);
+            ps = prof_begin(c, 4);
+            c->launches += launch_tile_stage_pre(c->g, c->q, c->k, fc, cstate(V, n), sg, cstate(Ua, n), state(out, n), c->src, c->ds, c->num_sms, c->stream);
+            prof_end(c, ps);
+            return MF_OK;
+        }
         if (!c->delta) {
             if (cudaMalloc(&c->delta, sizeof(double) * 5 * c->g.next) != cudaSuccess) { cudaGetLastError(); c->delta = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(delta) failed"); }
         }
@@ -154,7 +166,7 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
         }
         ps = prof_begin(c, 4);
         c->launches += launch_fused_stage(c->g, c->q, c->limiter, c->predictor, c->k, cstate(V, n), cstate(c->delta, c->g.next), sg, cstate(Ua, n),
-                                          state(out, n), c->src, c->ds, c->num_sms, c->sweep_variant, c->stream);
+                                          state(out, n), c->src, c->ds, c->num_sms, 0, c->stream);
         prof_end(c, ps);
     } else {
         int rc = ensure_staged_buffers(c);
@@ -168,7 +180,7 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
         c->launches += launch_flux_stage(c->g, c->q, c->k, 7, fc, fx, c->ds, c->stream);
         prof_end(c, ps);
         ps = prof_begin(c, 3);
-        c->launches += launch_combine(c->g, fx, sg, cstate(Ua, n), cstate(V, n), state(out, n), c->src, c->ds, c->stream);
+        c->launches += launch_combine(c->g, c->q, fx, sg, cstate(Ua, n), cstate(V, n), state(out, n), c->src, c->ds, c->stream);
         prof_end(c, ps);
     }
     return MF_OK;
@@ -184,6 +196,7 @@ int run_step(mf_ctx* c)
     if (c->rk == 2) {
         Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
         Stage s2 = { 1, 0.5, 0.5, 1.0, 1.0 };
+        s2.cfl = c->path == MF_PATH_STAGED;
         if ((rc = run_stage(c, Un, s1, Un, Ra)) != MF_OK) return rc;
         if ((rc = run_stage(c, Ra, s2, Un, Rb)) != MF_OK) return rc;
         c->cur = (c->cur + 2) % 3;
@@ -191,12 +204,14 @@ int run_step(mf_ctx* c)
         Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
         Stage s2 = { 2, 0.75, 0.25, 0.25, 1.0 };
         Stage s3 = { 2, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, 0.5 };
+        s3.cfl = c->path == MF_PATH_STAGED;
         if ((rc = run_stage(c, Un, s1, Un, Ra)) != MF_OK) return rc;
         if ((rc = run_stage(c, Ra, s2, Un, Rb)) != MF_OK) return rc;
         if ((rc = run_stage(c, Rb, s3, Un, Ra)) != MF_OK) return rc;
         c->cur = (c->cur + 1) % 3;
     }
     c->launches += launch_end_step(c->ds, c->stream);
+    c->smax_valid = c->path == MF_PATH_STAGED;
     return MF_OK;
 }
 
@@ -243,7 +258,7 @@ mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k
     if (!c) { fail(nullptr, MF_ENOMEM, "host allocation failed"); return nullptr; }
     memset(&c->g, 0, sizeof(c->g));
     c->U[0] = c->U[1] = c->U[2] = nullptr; c->faces = c->fluxes = nullptr; c->delta = nullptr;
-    { const char* v = getenv("MF_SWEEP_VARIANT"); c->sweep_variant = v ? atoi(v) : 0; } c->ds = nullptr; c->h_ds = nullptr;
+    c->ds = nullptr; c->h_ds = nullptr;
     c->partials = nullptr; c->h_partials = nullptr; c->own_stream = nullptr; c->stream = nullptr;
     cudaGetDevice(&c->dev);
     cudaDeviceProp prop;
@@ -270,7 +285,7 @@ mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k
     c->alpha = c->nact > 0 ? (double)c->nact : 1.0;                 // A9
     memset(&c->src, 0, sizeof(c->src));
     c->path_req = MF_PATH_AUTO; c->cur = 0; c->launches = 0;
-    c->prof_on = 0; c->prof_used = 0;
+    c->prof_on = 0; c->prof_used = 0; c->smax_valid = 0;
     resolve_path(c);
     c->nblocks_tot = c->num_sms * 4;
 
@@ -372,6 +387,7 @@ namespace {
 
 int reset_after_set(mf_ctx* c)
 {
+    c->smax_valid = 0;
     c->launches += launch_reset(c->ds, c->stream);
     return check_launch(c);
 }
@@ -468,9 +484,11 @@ int mf_step(mf_ctx* c, int n, double cfl)
     if (!c) return MF_EINVAL;
     if (n < 0 || !(cfl > 0.0)) return fail(c, MF_EINVAL, "bad n or cfl");
     for (int s = 0; s < n; ++s) {
-        int ps = prof_begin(c, 0);
-        c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->g.ncell), c->ds, c->num_sms, c->stream);   // a2, from U^n
-        prof_end(c, ps);
+        if (!c->smax_valid) {                                      // otherwise the previous step's last combine already reduced U^n
+            int ps = prof_begin(c, 0);
+            c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->g.ncell), c->ds, c->num_sms, c->stream);   // a2, from U^n
+            prof_end(c, ps);
+        }
         c->launches += launch_begin_step(c->ds, 0, cfl, c->g.dx, c->alpha, c->stream);
         int rc = run_step(c);
         if (rc != MF_OK) return rc;
@@ -498,6 +516,7 @@ int mf_eval_L(mf_ctx* c, double dt, double* L_E, double* L_Mx, double* L_My, dou
     double* scratch = c->U[(c->cur + 1) % 3];
     c->launches += launch_begin_step(c->ds, 1, dt, c->g.dx, c->alpha, c->stream);
     Stage sg = { 3, 0.0, 0.0, 0.0, 0.0 };
+    c->smax_valid = 0;
     Source keep = c->src;
     c->src.on = 0;
     int rc = run_stage(c, Un, sg, Un, scratch);
@@ -548,6 +567,7 @@ int mf_max_signal_speed(mf_ctx* c, double* smax)
     unsigned long long bits = c->h_ds->smax_bits;
     memcpy(smax, &bits, sizeof(double));
     // leave the accumulator empty for the next reduction
+    c->smax_valid = 0;
     cudaMemsetAsync(&c->ds->smax_bits, 0, sizeof(unsigned long long), c->stream);
     return rc;
 }
@@ -593,10 +613,10 @@ int mf_set_jet_source(mf_ctx* c, double dEdx, double sigma, double x0, double y0
 int mf_set_path(mf_ctx* c, int path)
 {
     if (!c) return MF_EINVAL;
-    if (path < MF_PATH_AUTO || path > MF_PATH_FUSED) return fail(c, MF_EINVAL, "unknown path");
+    if (path < MF_PATH_AUTO || path > MF_PATH_HYBRID) return fail(c, MF_EINVAL, "unknown path");
     int keep = c->path_req;
     c->path_req = path;
-    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "the fused path does not support this configuration"); }
+    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "the fused path does not support this configuration (it needs three active axes)"); }
     return MF_OK;
 }
 int mf_get_path(mf_ctx* c, int* path) { if (!c || !path) return MF_EINVAL; *path = c->path; return MF_OK; }

@@ -15,13 +15,19 @@ int launch_reset(StepState* ds, cudaStream_t st);
 // ---- staged path (MF_PATH_STAGED): a3+a4, a5, a7(+a8) as three kernels, face states and fluxes through HBM
 int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, CState5 V, Faces fc, const StepState* ds, cudaStream_t st);
 int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask /* bit d: compute direction d */, Faces fc, Fluxes fx, const StepState* ds, cudaStream_t st);
-int launch_combine(const Grid& g, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, const StepState* ds, cudaStream_t st);
+int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds, cudaStream_t st);   // sg.cfl: + a2
 
 // ---- fused path (MF_PATH_FUSED): one kernel per RK stage
 bool fused_supported(const Grid& g);
 int launch_delta_stage(const Grid& g, const Eos& q, int limiter, CState5 V, State5 D, const StepState* ds, cudaStream_t st);
 int launch_fused_stage(const Grid& g, const Eos& q, int limiter, int predictor, int k, CState5 V, CState5 D, Stage sg, CState5 Ua,
                        State5 out, Source src, const StepState* ds, int num_sms, int variant, cudaStream_t st);
+
+int launch_tile_stage(const Grid& g, const Eos& q, int limiter, int predictor, int k, CState5 V, CState5 D, Stage sg, CState5 Ua, State5 out,
+                      Source src, const StepState* ds, int num_sms, cudaStream_t st);
+
+int launch_tile_stage_pre(const Grid& g, const Eos& q, int k, Faces fc, CState5 V, Stage sg, CState5 Ua, State5 out, Source src,
+                          const StepState* ds, int num_sms, cudaStream_t st);
 
 // ---- conversions and reductions
 int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st);          // in place: (e,v,n) -> (E,M,R), Eq.4

@@ -58,6 +58,7 @@ struct Fluxes {
 struct Stage {
     int form;        // 0: Ua + dt*L   1: 0.5*(Ua + Ub + dt*L)   2: ca*Ua + cb*Ub + (cdt*dt)*L
     double ca, cb, cdt, ts;
+    int cfl;         // 1: this is the step's last stage: also reduce S_max / status of the new state for the next step (a2)
 };
 
 } // namespace mf
