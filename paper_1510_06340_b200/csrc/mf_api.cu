@@ -176,12 +176,22 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
         int ps = prof_begin(c, 1);
         c->launches += launch_cell_stage(c->g, c->q, c->limiter, c->predictor, cstate(V, n), fc, c->ds, c->stream);
         prof_end(c, ps);
-        ps = prof_begin(c, 2);
-        c->launches += launch_flux_stage(c->g, c->q, c->k, 7, fc, fx, c->ds, c->stream);
-        prof_end(c, ps);
-        ps = prof_begin(c, 3);
-        c->launches += launch_combine(c->g, c->q, fx, sg, cstate(Ua, n), cstate(V, n), state(out, n), c->src, c->ds, c->stream);
-        prof_end(c, ps);
+        if (c->g.act[0]) {
+            // y and z fluxes to HBM, then the x fluxes fused with divergence + source + RK combine (F_x stays on chip)
+            ps = prof_begin(c, 2);
+            c->launches += launch_flux_stage(c->g, c->q, c->k, 6, fc, fx, c->ds, c->stream);
+            prof_end(c, ps);
+            ps = prof_begin(c, 3);
+            c->launches += launch_xflux_combine(c->g, c->q, c->k, fc, fx, sg, cstate(Ua, n), cstate(V, n), state(out, n), c->src, c->ds, c->stream);
+            prof_end(c, ps);
+        } else {
+            ps = prof_begin(c, 2);
+            c->launches += launch_flux_stage(c->g, c->q, c->k, 7, fc, fx, c->ds, c->stream);
+            prof_end(c, ps);
+            ps = prof_begin(c, 3);
+            c->launches += launch_combine(c->g, c->q, fx, sg, cstate(Ua, n), cstate(V, n), state(out, n), c->src, c->ds, c->stream);
+            prof_end(c, ps);
+        }
     }
     return MF_OK;
 }

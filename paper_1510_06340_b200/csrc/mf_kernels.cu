@@ -7,7 +7,10 @@ namespace mf {
 
 constexpr int TPB = 256;
 #ifndef MF_CELL_MINB
-#define MF_CELL_MINB 2
+#define MF_CELL_MINB 3
+#endif
+#ifndef MF_FLUX_MINB
+#define MF_FLUX_MINB 3
 #endif
 
 static inline unsigned int blocks_for(long long n, int tpb) { return (unsigned int)((n + tpb - 1) / tpb); }
@@ -254,7 +257,7 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
 // =========================================================================== a5 + a6: interface fluxes
 // One thread per interface between cell c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
 template <int D>
-__global__ void __launch_bounds__(TPB, 3) k_flux_stage(Grid g, Eos q, int k, Faces fc, Fluxes fx, const StepState* ds)
+__global__ void __launch_bounds__(TPB, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, int k, Faces fc, Fluxes fx, const StepState* ds)
 {
     int m[3] = { g.n[0], g.n[1], g.n[2] };
     m[D] += 1;
@@ -363,6 +366,79 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
 int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds, cudaStream_t st)
 {
     k_combine<<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+    return 1;
+}
+
+// =========================================================================== a5 (x) + a7 + a8 (+ a2) in one kernel
+// The x fluxes are the last ones of a stage.  Thread t of a block owns x interface I = 255*block + t (linear over all rows, nx+1 per
+// row), runs MUSTA on it and leaves the flux in shared memory; the cell to the right of the interface then has both of its x fluxes on
+// chip (its own and thread t+1's), reads F_y, F_z of its four other faces, and is finished: divergence, source, RK combine, one store.
+// Blocks overlap by one interface, so 255 of 256 threads finish a cell.  F_x is never written, and the 40 loads of the combine hide
+// under the FP64 work of a compute-bound kernel instead of making a memory-bound pass of their own.
+// 64 registers / 4 blocks per SM: measured on B200, 32 resident warps let the combine's loads of one block overlap the MUSTA of the
+// others (1.37 ms per launch at 256^3 against 1.56 ms at 24 warps; prefetching the operands with cp.async into shared memory at 24
+// warps did not help, 1.53 ms: the kernel is then limited by DRAM bandwidth, not by latency).
+__global__ void __launch_bounds__(TPB, 4) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
+                                                          Source src, StepState* ds)
+{
+    __shared__ double sF[5][TPB];
+    const int t = threadIdx.x;
+    const int nf = g.n[0] + 1;                                              // x interfaces per row
+    const long long nrows = (long long)g.n[1] * g.n[2];
+    const long long I = (long long)blockIdx.x * (TPB - 1) + t;
+    const bool live = I < nrows * nf;
+    int f = 0, j = 0, kz = 0;
+    long long p = 0;
+    double F[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
+    if (live) {
+        const long long r = I / nf;
+        f = (int)(I - r * nf);                                              // interface between cells f-1 and f of the row
+        j = (int)(r % g.n[1]); kz = (int)(r / g.n[1]);
+        p = f + (long long)(j + g.h[1]) * g.es[1] + (long long)(kz + g.h[2]) * g.es[2];    // extended index of cell f-1
+        double A[5], B[5];
+#ifdef MF_STRICT
+#pragma unroll
+        for (int v = 0; v < 5; ++v) { A[v] = fc.f[0][1][v][p]; B[v] = fc.f[0][0][v][p + 1]; }
+#else
+#pragma unroll
+        for (int v = 0; v < 5; ++v) { A[v] = fc.f[0][1][v][p] + fc.f[0][0][v][p]; B[v] = fc.f[0][1][v][p + 1] - fc.f[0][0][v][p + 1]; }
+#endif
+        musta_flux<0>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
+    }
+#pragma unroll
+    for (int v = 0; v < 5; ++v) sF[v][t] = F[v];
+    __syncthreads();
+    double smax = 0.0;
+    int bad = 0;
+    if (live && t < TPB - 1 && f < g.n[0]) {                                // cell (f, j, kz): lower x face = this interface, upper = thread t+1's
+        const long long pc = p + 1;
+        const long long o = f + (long long)j * g.ns[1] + (long long)kz * g.ns[2];
+        const double dt = ds->dt;
+        double S = 0.0;
+        if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
+        double W[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+            double acc = sF[v][t + 1] - F[v];
+            if (g.act[1]) acc = acc + (fx.f[1][v][pc] - fx.f[1][v][pc - g.es[1]]);
+            if (g.act[2]) acc = acc + (fx.f[2][v][pc] - fx.f[2][v][pc - g.es[2]]);
+            double L = -acc / g.dx;                                        // Eq.1 :43
+            if (src.on && v < 2) L = L + S;
+            double ua = sg.form == 3 ? 0.0 : Ua.q[v][o];
+            double ub = (sg.form == 1 || sg.form == 2) ? Ub.q[v][o] : 0.0;
+            W[v] = rk_form(sg, ua, ub, dt, L);
+            out.q[v][o] = W[v];
+        }
+        if (sg.cfl) smax = signal_speed(q, W[0], W[1], W[2], W[3], W[4], bad);
+    }
+    if (sg.cfl) block_reduce_smax(smax, bad, ds);
+}
+
+int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src,
+                         StepState* ds, cudaStream_t st)
+{
+    const long long total = (long long)(g.n[0] + 1) * g.n[1] * g.n[2];
+    k_xflux_combine<<<blocks_for(total, TPB - 1), TPB, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds);
     return 1;
 }
 

@@ -17,6 +17,10 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
 int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask /* bit d: compute direction d */, Faces fc, Fluxes fx, const StepState* ds, cudaStream_t st);
 int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds, cudaStream_t st);   // sg.cfl: + a2
 
+// x fluxes fused with divergence + source + RK combine (+ a2 when sg.cfl); F_y, F_z must already be in fx (needs an active x axis)
+int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src,
+                         StepState* ds, cudaStream_t st);
+
 // ---- fused path (MF_PATH_FUSED): one kernel per RK stage
 bool fused_supported(const Grid& g);
 int launch_delta_stage(const Grid& g, const Eos& q, int limiter, CState5 V, State5 D, const StepState* ds, cudaStream_t st);
