@@ -51,12 +51,37 @@ def alg_slots(limiter, k, rk, ndim, predictor=True):
     return rk * per_L + cfl, per_L, ndim * musta
 
 
+def class_work(path, limiter, k, ndim, x_active, predictor=True):
+    """Algorithmic (FP64 slots, HBM bytes) per cell of one launch group of each kernel class, for one RK stage.
+    Bytes are what that kernel must read and write given the data layout of DESIGN.md section 4."""
+    recon = 5 * ndim * (4 + SLOPE[limiter])
+    pred = (2 * ndim * FLUX + 5 * 4 * ndim) if predictor else 0
+    musta = (k + 1) * (3 * FLUX + 50) + 20 * k
+    comb = 5 * (2 * ndim + 5)
+    if path == "staged":
+        nflux = ndim - 1 if x_active else ndim
+        out = {"cell_stage": (recon + pred, 40 + 40 * (1 + ndim)),            # U in; W and the half slopes H_d out
+               "flux_stage": (nflux * musta, nflux * 120)}                    # W, H_d in, F_d out, per direction
+        if x_active:
+            out["combine"] = (musta + comb, 80 + 40 * (ndim - 1) + 80 + 40)   # W, H_x, F_y, F_z, U^n, U_(s) in; new state out
+        else:
+            out["combine"] = (comb, 40 * ndim + 80 + 40)
+        return out
+    if path == "hybrid":
+        return {"cell_stage": (recon + pred, 40 + 40 * (1 + ndim)), "fused_stage": (ndim * musta + comb, 40 + 40 * ndim + 80 + 40)}
+    return {"cell_stage": (recon + pred, 80), "fused_stage": (recon + ndim * musta + comb, 80 + 80 + 40)}   # fused: delta kernel + tile kernel
+
+
 def alg_bytes(rk):
     """Minimum HBM bytes per cell-update: stage 1 reads U^n writes U1 (80 B), later stages read U_s and U^n, write (120 B); CFL +32 B."""
     return 80 + 120 * (rk - 1) + 32
 
 
-FP64_LANES_PER_SM = 64        # B200 (sm_100): 4 SMSPs x 16 FP64 lanes; mf_probe_fp64 measures it (DESIGN.md)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch group at 256^3 (config 3, staged path), one ncu --set full capture:
+# k_cell_stage 0.683 + 2.709 GB; k_flux_stage<1>, <2> 2.033 + 2.034 GB; k_xflux_combine 4.097 + 0.817 GB (profiles/r01_ncu_full_staged_256.md)
+NCU_TRAFFIC_GB_256 = {"cell_stage": 3.392, "flux_stage": 4.067, "combine": 4.914}
+
+FP64_LANES_PER_SM = 64       # B200 (sm_100): 4 SMSPs x 16 FP64 lanes; mf_probe_fp64 measures it (DESIGN.md)
 
 
 def peaks():
@@ -278,16 +303,32 @@ def run_ours(args):
     slots_cu, slots_L, slots_musta = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim)
     alu_peak_slots = 148 * FP64_LANES_PER_SM * pk["sm_max_mhz"] * 1e6          # FP64 instructions/s, all SMs
     # dominant kernel, from the event pairs recorded around every launch inside the timed region
-    dom = max((k for k in prof if k in ("fused_stage", "flux_stage")), key=lambda k: prof[k][0], default=None)
-    roof = None
-    if dom:
-        ms, groups = prof[dom]
-        per_launch_slots = (slots_L if dom == "fused_stage" else slots_musta) * cells
-        achieved = 2.0 * per_launch_slots / (ms / groups * 1e-3) / 1e12
-        peak = 2.0 * alu_peak_slots / 1e12
-        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
-                "kernel": dom, "launch_ms": ms / groups, "share_of_step": ms / elapsed_ms,
-                "note": "FMA-equivalent flops = 2 x algorithmic FP64 issue slots (div = sqrt = 8 slots); peak = 2 x 148 SM x 64 lanes x clocks.max.sm"}
+    work = class_work(g.path(), sch["limiter"], sch["k_stages"], ndim, nx > 1)
+    kernels = {}
+    for name, (ms, groups) in prof.items():
+        if name not in work or groups == 0:
+            continue
+        slots, nbytes = work[name]
+        t = ms / groups * 1e-3                                              # one launch group = this class's launches of one RK stage
+        t_alu, t_hbm = slots * cells / alu_peak_slots, nbytes * cells / (pk["hbm_gbs"] * 1e9)
+        if t_alu >= t_hbm:
+            ach, peak, unit, bound = 2.0 * slots * cells / t / 1e12, 2.0 * alu_peak_slots / 1e12, "TFLOP/s", "alu"
+        else:
+            ach, peak, unit, bound = nbytes * cells / t / 1e9, pk["hbm_gbs"], "GB/s", "hbm"
+        kernels[name] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak, "traffic": None,
+                         "kernel": name, "launch_ms": ms / groups, "share_of_step": ms / elapsed_ms,
+                         "alg_slots_per_cell": slots, "alg_bytes_per_cell": nbytes}
+    # DRAM traffic per launch group from the committed ncu --set full capture of this same workload (profiles/r01_ncu_full_staged_256.md)
+    if g.path() == "staged" and (nx, ny, nz) == (256, 256, 256) and sch["k_stages"] == 3 and sch["rk"] == 3:
+        for name, gb in NCU_TRAFFIC_GB_256.items():
+            if name in kernels:
+                kernels[name]["traffic"] = gb * 1e9
+    # the dominant kernel class = the one with the largest share of the timed region
+    roof = max(kernels.values(), key=lambda r: r["share_of_step"]) if kernels else None
+    if roof:
+        roof = dict(roof, note="alu: FMA-equivalent flops = 2 x algorithmic FP64 issue slots (div = sqrt = 8 slots), peak = 2 x 148 SM x 64 "
+                               "lanes x clocks.max.sm; hbm: algorithmic bytes of that kernel / measured copy bandwidth; launch_ms is one "
+                               "launch group (the class's launches of one RK stage) from CUDA-event pairs on the library's stream")
     step_frac_alu = (slots_cu * cells * args.steps / (elapsed_ms * 1e-3)) / alu_peak_slots
     step_frac_hbm = (alg_bytes(sch["rk"]) * cells * args.steps / (elapsed_ms * 1e-3)) / (pk["hbm_gbs"] * 1e9)
     probe = binding.probe_fp64()
@@ -302,6 +343,7 @@ def run_ours(args):
                     "steps": e2e_steps, "note": "mf_set_state(host) + mf_step(1) + mf_get_state(host) per step, pinned host buffers"},
             "gpu_launches": launches,
             "roofline": roof,
+            "roofline_kernels": kernels,
             "roofline_step": {"alg_slots_per_cell_update": slots_cu, "alg_bytes_per_cell_update": alg_bytes(sch["rk"]),
                               "frac_alu": step_frac_alu, "frac_hbm": step_frac_hbm, "hbm_peak": pk["hbm_source"],
                               "measured_dfma_per_s": probe["dfma_per_s"], "measured_rcp_slots": probe["dfma_per_s"] / probe["rcp_per_s"],

@@ -403,6 +403,16 @@ __global__ void __launch_bounds__(TPB, 4) k_xflux_combine(Grid g, Eos q, int k, 
 #pragma unroll
         for (int v = 0; v < 5; ++v) { A[v] = fc.f[0][1][v][p] + fc.f[0][0][v][p]; B[v] = fc.f[0][1][v][p + 1] - fc.f[0][0][v][p + 1]; }
 #endif
+        if (t < TPB - 1 && f < g.n[0]) {                                    // pull the combine's operands towards L2 while MUSTA runs
+            const long long pc = p + 1, o = f + (long long)j * g.ns[1] + (long long)kz * g.ns[2];
+#pragma unroll
+            for (int v = 0; v < 5; ++v) {
+                if (g.act[1]) prefetch_l2(&fx.f[1][v][pc]);      // the neighbour lines (pc - es) are somebody else's pc: prefetching
+                if (g.act[2]) prefetch_l2(&fx.f[2][v][pc]);      // them too measured slower
+                if (sg.form != 3) prefetch_l2(&Ua.q[v][o]);
+                if (sg.form == 1 || sg.form == 2) prefetch_l2(&Ub.q[v][o]);
+            }
+        }
         musta_flux<0>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
     }
 #pragma unroll
