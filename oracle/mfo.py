@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 
 LIM = {"none": 0, "minmod": 1, "superbee": 2, "vanalbada": 3, "vanleer": 4, "mc": 5, "first": 6}
 BC = {"outflow": 0, "periodic": 1}
-EOS_CS2 = 0
+EOS_CS2, EOS_TABLE = 0, 1
 OK, EINVAL, ENOMEM, ESTATE = 0, -1, -2, -4
 
 _dp = C.POINTER(C.c_double)
@@ -48,6 +48,8 @@ def _load(omp):
         "mfo_set_predictor": (C.c_int, [vp, C.c_int]),
         "mfo_set_alpha": (C.c_int, [vp, C.c_double]),
         "mfo_set_jet_source": (C.c_int, [vp] + [C.c_double] * 5),
+        "mfo_set_eos_table": (C.c_int, [vp, C.c_int, C.c_int] + [C.c_double] * 4 + [_dp]),
+        "mfo_eos": (C.c_int, [vp, C.c_double, C.c_double, _dp]),
         "mfo_sync": (C.c_int, [vp]),
         "mfo_last_error": (C.c_char_p, [vp]),
         "mfo_slope": (C.c_double, [C.c_int, C.c_double, C.c_double]),
@@ -85,12 +87,12 @@ class Oracle:
     """One oracle context.  Arrays are numpy float64 of shape (nz, ny, nx) (x fastest) or flat."""
 
     def __init__(self, nx, ny=1, nz=1, dx=1.0, limiter="minmod", k_stages=2, rk=2, bc="outflow",
-                 predictor=True, alpha=None, cs2=None, omp=False):
+                 predictor=True, alpha=None, cs2=None, omp=False, eos_table=None):
         self.lib = _load(omp)
         self.shape = (nz, ny, nx)
         self.n = nx * ny * nz
         lim = LIM[limiter] if isinstance(limiter, str) else int(limiter)
-        self.h = self.lib.mfo_create(nx, ny, nz, float(dx), EOS_CS2, lim, int(k_stages))
+        self.h = self.lib.mfo_create(nx, ny, nz, float(dx), EOS_CS2 if eos_table is None else EOS_TABLE, lim, int(k_stages))
         if not self.h:
             raise OracleError("mfo_create failed (bad arguments)")
         self._chk(self.lib.mfo_set_rk(self.h, int(rk)))
@@ -100,6 +102,8 @@ class Oracle:
             self._chk(self.lib.mfo_set_alpha(self.h, float(alpha)))
         if cs2 is not None:
             self._chk(self.lib.mfo_set_cs2(self.h, float(cs2)))
+        if eos_table is not None:
+            self.set_eos_table(eos_table)
 
     def _chk(self, rc, allow=()):
         if rc != OK and rc not in allow:
@@ -154,6 +158,17 @@ class Oracle:
 
     def set_jet_source(self, dEdx, sigma, x0, y0, z0):
         self._chk(self.lib.mfo_set_jet_source(self.h, dEdx, sigma, x0, y0, z0))
+
+    def set_eos_table(self, tb):
+        """tb: dict(ln_e0, dln_e, n0, dn, ln_p) with ln_p of shape (nn, ne) (see workloads.crossover_eos_table)."""
+        ln_p = _f64(tb["ln_p"])
+        nn, ne = (1, ln_p.size) if ln_p.ndim == 1 else ln_p.shape
+        self._chk(self.lib.mfo_set_eos_table(self.h, ne, nn, tb["ln_e0"], tb["dln_e"], tb.get("n0", 0.0), tb.get("dn", 1.0), _p(ln_p)))
+
+    def eos(self, e, n=0.0):
+        out = np.empty(3)
+        self._chk(self.lib.mfo_eos(self.h, float(e), float(n), _p(out)))
+        return out
 
     def status(self):
         return self.lib.mfo_sync(self.h)

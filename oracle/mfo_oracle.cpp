@@ -42,9 +42,55 @@ namespace {
 const double E_VACUUM = 1e-12;          /* A12(i)  */
 const double V_CAP    = 1.0 - 1e-10;    /* A12(ii) */
 
+/* Equation of state p = p(e, n), Eq.2 PAPER.md:47.  kind 0: p = cs2*e (the only one the paper gives concretely, :312).
+ * kind 1: tabulated.  ln p is stored on a grid that is uniform in ln e (ne points from ln_e0, step dln_e) and uniform in n
+ * (nn points from n0, step dn; nn = 1 means no n dependence) and interpolated bilinearly; below/above the e range the end
+ * cells extrapolate linearly in (ln e, ln p), outside the n range the value is held.  DESIGN.md reading A18. */
 struct Params {
     double cs2;
+    int kind;
+    int ne, nn;
+    double ln_e0, dln_e, n0, dn;
+    const double* lnp;          /* [nn][ne], e fastest */
 };
+
+struct EosValue {
+    double p, p_e, p_n;         /* p, dp/de at fixed n, dp/dn at fixed e */
+};
+
+EosValue eos_eval(const Params& P, double e, double n)
+{
+    EosValue r;
+    if (P.kind == 0) { r.p = P.cs2 * e; r.p_e = P.cs2; r.p_n = 0.0; return r; }
+    double x = (std::log(e) - P.ln_e0) / P.dln_e;
+    int i = (int)std::floor(x);
+    if (i < 0) i = 0;
+    if (i > P.ne - 2) i = P.ne - 2;
+    double fx = x - (double)i;                          /* may leave [0,1]: linear extrapolation in (ln e, ln p) */
+    int j = 0;
+    double fy = 0.0;
+    bool n_inside = false;
+    if (P.nn > 1) {
+        double y = (n - P.n0) / P.dn;
+        j = (int)std::floor(y);
+        if (j < 0) j = 0;
+        if (j > P.nn - 2) j = P.nn - 2;
+        fy = y - (double)j;
+        n_inside = fy >= 0.0 && fy <= 1.0;
+        if (fy < 0.0) fy = 0.0;
+        if (fy > 1.0) fy = 1.0;
+    }
+    const double* row0 = P.lnp + (long)j * P.ne;
+    const double* row1 = P.nn > 1 ? row0 + P.ne : row0;
+    double d0 = row0[i + 1] - row0[i], d1 = row1[i + 1] - row1[i];
+    double l0 = row0[i] + fx * d0, l1 = row1[i] + fx * d1;
+    double lp = l0 + fy * (l1 - l0);
+    r.p = std::exp(lp);
+    double dlnp_dlne = ((1.0 - fy) * d0 + fy * d1) / P.dln_e;
+    r.p_e = r.p * dlnp_dlne / e;
+    r.p_n = n_inside ? r.p * ((l1 - l0) / P.dn) : 0.0;
+    return r;
+}
 
 /* ---------- Eq.14-21 in two-argument form (reading A6/A7/A8): a = U_i-U_{i-1}, b = U_{i+1}-U_i ---------- */
 double slope2(int lim, double a, double b)
@@ -92,9 +138,38 @@ double slope2(int lim, double a, double b)
 /* ---------- Eq.23 for p = cs2*e in closed form, with the admissibility guard A12 ----------
  * v = M/(E+p), e = E - M.v, p = cs2*e  =>  |v| = 2|M| / ((1+cs2)E + sqrt((1+cs2)^2 E^2 - 4 cs2 |M|^2)).
  * Returns v (3), e, p.  PAPER.md:227-234. */
-void velocity_pressure(double cs2, double E, double Mx, double My, double Mz,
+/* Eq.23 for a general p(e, n): the last line is a scalar equation for the speed v = |v|,
+ *     f(v) = v (E + p(E - |M| v, R sqrt(1 - v^2))) - |M| = 0,
+ * solved by Newton's method from v = |M|/E (where f >= 0), kept inside a bracket [lo, hi] by bisection whenever a Newton step
+ * leaves it; at most 60 iterations, stop when |dv| <= 1e-15.  The paper says "solved numerically ... as the fixed point
+ * equation for v" (:236); BASELINE.json's north_star names Newton.  DESIGN.md reading A18.  Returns the speed. */
+double solve_speed(const Params& P, double E, double M, double R, double* e_out, double* p_out)
+{
+    double lo = 0.0, hi = M / E, v = hi;
+    for (int it = 0; it < 60; ++it) {
+        double e = E - M * v;
+        double g = std::sqrt(1.0 - v * v);
+        EosValue q = eos_eval(P, e, R * g);
+        double f = v * (E + q.p) - M;
+        if (f == 0.0) break;
+        if (f > 0.0) hi = v; else lo = v;
+        double df = E + q.p + v * (-M * q.p_e - R * (v / g) * q.p_n);
+        double vn = v - f / df;
+        if (!(vn > lo && vn < hi)) vn = 0.5 * (lo + hi);
+        double dv = std::fabs(vn - v);
+        v = vn;
+        if (dv <= 1e-15) break;
+    }
+    double e = E - M * v;
+    *e_out = e;
+    *p_out = eos_eval(P, e, R * std::sqrt(1.0 - v * v)).p;
+    return v;
+}
+
+void velocity_pressure(const Params& P, double E, double Mx, double My, double Mz, double R,
                        double v[3], double* e_out, double* p_out)
 {
+    const double cs2 = P.cs2;
     if (!(E > E_VACUUM)) {                               /* A12(i): vacuum -> v = 0, p = 0 (NaN E also lands here) */
         if (E != E) { v[0] = v[1] = v[2] = E; *e_out = E; *p_out = E; return; }
         v[0] = v[1] = v[2] = 0.0; *e_out = E; *p_out = 0.0;
@@ -107,6 +182,19 @@ void velocity_pressure(double cs2, double E, double Mx, double My, double Mz,
         Mx *= s; My *= s; Mz *= s;
         M2 = Mx * Mx + My * My + Mz * Mz;
     }
+    if (P.kind != 0) {                                   /* tabulated EOS: Newton on the speed, then v_j = M_j v/|M| */
+        double M = std::sqrt(M2);
+        if (M == 0.0) {
+            v[0] = v[1] = v[2] = 0.0; *e_out = E; *p_out = eos_eval(P, E, R).p;
+            return;
+        }
+        double e, p;
+        double sp = solve_speed(P, E, M, R, &e, &p);
+        double s = sp / M;
+        v[0] = Mx * s; v[1] = My * s; v[2] = Mz * s;
+        *e_out = e; *p_out = p;
+        return;
+    }
     double c1 = 1.0 + cs2;
     double Q = std::sqrt(c1 * c1 * E * E - 4.0 * cs2 * M2);
     double inv = 2.0 / (c1 * E + Q);
@@ -117,10 +205,10 @@ void velocity_pressure(double cs2, double E, double Mx, double My, double Mz,
 }
 
 /* ---------- Eq.3: F_d(U) = ((E+p)v_d, M_j v_d + p delta_jd, R v_d) ---------- */
-void flux_d(double cs2, int d, const double U[5], double F[5])
+void flux_d(const Params& P, int d, const double U[5], double F[5])
 {
     double v[3], e, p;
-    velocity_pressure(cs2, U[0], U[1], U[2], U[3], v, &e, &p);
+    velocity_pressure(P, U[0], U[1], U[2], U[3], U[4], v, &e, &p);
     double vd = v[d];
     F[0] = (U[0] + p) * vd;
     F[1] = U[1] * vd;
@@ -134,7 +222,7 @@ void flux_d(double cs2, int d, const double U[5], double F[5])
  * A = U_L^(0), B = U_R^(0).  c_lw = 0.5*alpha*lam, c_lf = 0.5/(alpha*lam) (computed once per step, A16).
  * Reading A1: the Lax-Wendroff state of Eq.10 uses the FLUX difference (Richtmyer), not U_R-U_L as printed.
  * Reading A5: k = number of Eq.8 updates; FORCE is evaluated k+1 times. */
-void musta_flux(double cs2, int d, int k, double lam, double c_lw, double c_lf,
+void musta_flux(const Params& cs2, int d, int k, double lam, double c_lw, double c_lf,
                 const double A0[5], const double B0[5], double F[5])
 {
     double A[5], B[5], FA[5], FB[5], Ulw[5], Flw[5], Flf[5];
@@ -165,7 +253,9 @@ struct mfo_ctx {
     int nact;
     double dx;
     int eos, limiter, k, rk, bc, predictor;
-    double cs2, alpha;
+    Params P;
+    std::vector<double> table;   /* owned copy of ln p for the tabulated EOS */
+    double alpha;
     double jet_dEdx, jet_sigma, jet_x0[3];
     double t, last_dt;
     long long steps;
@@ -218,7 +308,7 @@ void eval_L(mfo_ctx* c, const std::vector<double> V[5], double dt)
     const double hl = 0.5 * lam;
     const double c_lw = 0.5 * c->alpha * lam;
     const double c_lf = 0.5 / (c->alpha * lam);
-    const double cs2 = c->cs2;
+    const Params& cs2 = c->P;
 
     fill_with_ghosts(c, V);
 
@@ -342,7 +432,6 @@ void rk_combine(mfo_ctx* c, std::vector<double> out[5], double ca, const std::ve
 /* a2: S_max = max_cells (|v|+cs)/(1+|v|cs), |v| from Eq.23.  Not in the paper (fixed dt there); reading A10. */
 double max_signal_speed(mfo_ctx* c, int* bad)
 {
-    double cs = std::sqrt(c->cs2);
     double smax = 0.0;
     int nbad = 0;
     for (long o = 0; o < c->ncell; ++o) {
@@ -350,8 +439,18 @@ double max_signal_speed(mfo_ctx* c, int* bad)
         if (!std::isfinite(E) || !std::isfinite(Mx) || !std::isfinite(My) || !std::isfinite(Mz) || !std::isfinite(R)) { ++nbad; continue; }
         if (E > E_VACUUM && Mx * Mx + My * My + Mz * Mz > E * E) ++nbad;   /* superluminal stored state (guard still applies) */
         double v[3], e, p;
-        velocity_pressure(c->cs2, E, Mx, My, Mz, v, &e, &p);
+        velocity_pressure(c->P, E, Mx, My, Mz, R, v, &e, &p);
         double av = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+        double cs = std::sqrt(c->P.cs2);
+        if (c->P.kind != 0) {                               /* adiabatic sound speed of the table: cs^2 = p_e + n p_n/(e+p) */
+            double cs2t = 0.0;
+            if (e > 0.0) {
+                double nn = R * std::sqrt(1.0 - av * av);
+                EosValue q = eos_eval(c->P, e, nn);
+                cs2t = q.p_e + nn * q.p_n / (e + q.p);
+            }
+            cs = cs2t > 0.0 ? std::sqrt(cs2t) : 0.0;
+        }
         double s = (av + cs) / (1.0 + av * cs);
         if (s > smax) smax = s;
     }
@@ -390,7 +489,7 @@ mfo_ctx* mfo_create(int nx, int ny, int nz, double dx, int eos, int limiter, int
 {
     const int n[3] = { nx, ny, nz };
     for (int a = 0; a < 3; ++a) if (n[a] < 1 || (n[a] > 1 && n[a] < 4)) return nullptr;
-    if (!(dx > 0.0) || eos != MFO_EOS_CS2 || limiter < 0 || limiter > MFO_LIM_FIRST || k_stages < 0 || k_stages > 8) return nullptr;
+    if (!(dx > 0.0) || (eos != MFO_EOS_CS2 && eos != MFO_EOS_TABLE) || limiter < 0 || limiter > MFO_LIM_FIRST || k_stages < 0 || k_stages > 8) return nullptr;
     mfo_ctx* c = new (std::nothrow) mfo_ctx();
     if (!c) return nullptr;
     c->nact = 0;
@@ -401,7 +500,8 @@ mfo_ctx* mfo_create(int nx, int ny, int nz, double dx, int eos, int limiter, int
     c->ncell = (long)nx * ny * nz;
     c->ntot = (long)c->tot[0] * c->tot[1] * c->tot[2];
     c->dx = dx; c->eos = eos; c->limiter = limiter; c->k = k_stages;
-    c->rk = 2; c->bc = MFO_BC_OUTFLOW; c->predictor = 1; c->cs2 = 1.0 / 3.0;
+    c->rk = 2; c->bc = MFO_BC_OUTFLOW; c->predictor = 1;
+    c->P.cs2 = 1.0 / 3.0; c->P.kind = 0; c->P.ne = c->P.nn = 0; c->P.ln_e0 = c->P.dln_e = c->P.n0 = c->P.dn = 0.0; c->P.lnp = nullptr;
     c->alpha = c->nact > 0 ? (double)c->nact : 1.0;         /* A9: alpha = number of active directions */
     c->jet_dEdx = 0.0; c->jet_sigma = 1.0; c->jet_x0[0] = c->jet_x0[1] = c->jet_x0[2] = 0.0;
     c->t = 0.0; c->last_dt = 0.0; c->steps = 0; c->status = MFO_OK;
@@ -443,7 +543,7 @@ int mfo_prim2con(mfo_ctx* c, const double prim[5], double U[5])
     if (!c || !prim || !U) return MFO_EINVAL;
     /* Eq.4: E=(eps+p)g^2-p, M_i=(eps+p)g^2 v_i, R=n g, g=1/sqrt(1-v^2) */
     double e = prim[0], vx = prim[1], vy = prim[2], vz = prim[3], nn = prim[4];
-    double p = c->cs2 * e;
+    double p = eos_eval(c->P, e, nn).p;
     double g2 = 1.0 / (1.0 - (vx * vx + vy * vy + vz * vz));
     double w = (e + p) * g2;
     U[0] = w - p; U[1] = w * vx; U[2] = w * vy; U[3] = w * vz; U[4] = nn * std::sqrt(g2);
@@ -454,7 +554,7 @@ int mfo_con2prim(mfo_ctx* c, const double U[5], double prim[5])
 {
     if (!c || !prim || !U) return MFO_EINVAL;
     double v[3], e, p;
-    velocity_pressure(c->cs2, U[0], U[1], U[2], U[3], v, &e, &p);
+    velocity_pressure(c->P, U[0], U[1], U[2], U[3], U[4], v, &e, &p);
     prim[0] = e; prim[1] = v[0]; prim[2] = v[1]; prim[3] = v[2];
     prim[4] = U[4] * std::sqrt(1.0 - (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));   /* n = R sqrt(1-v^2), Eq.23 */
     return MFO_OK;
@@ -540,7 +640,7 @@ int mfo_get_time(mfo_ctx* c, double* t, double* last_dt, long long* steps)
 
 int mfo_set_rk(mfo_ctx* c, int order) { if (!c) return MFO_EINVAL; if (order != 2 && order != 3) return fail(c, MFO_EINVAL, "rk order must be 2 or 3"); c->rk = order; return MFO_OK; }
 int mfo_set_boundary(mfo_ctx* c, int bc) { if (!c) return MFO_EINVAL; if (bc != MFO_BC_OUTFLOW && bc != MFO_BC_PERIODIC) return fail(c, MFO_EINVAL, "unknown bc"); c->bc = bc; return MFO_OK; }
-int mfo_set_cs2(mfo_ctx* c, double cs2) { if (!c) return MFO_EINVAL; if (!(cs2 > 0.0) || !(cs2 < 1.0)) return fail(c, MFO_EINVAL, "cs2 must be in (0,1)"); c->cs2 = cs2; return MFO_OK; }
+int mfo_set_cs2(mfo_ctx* c, double cs2) { if (!c) return MFO_EINVAL; if (!(cs2 > 0.0) || !(cs2 < 1.0)) return fail(c, MFO_EINVAL, "cs2 must be in (0,1)"); c->P.cs2 = cs2; return MFO_OK; }
 int mfo_set_predictor(mfo_ctx* c, int on) { if (!c) return MFO_EINVAL; c->predictor = on ? 1 : 0; return MFO_OK; }
 int mfo_set_alpha(mfo_ctx* c, double alpha) { if (!c) return MFO_EINVAL; if (!(alpha > 0.0)) return fail(c, MFO_EINVAL, "alpha must be > 0"); c->alpha = alpha; return MFO_OK; }
 int mfo_set_jet_source(mfo_ctx* c, double dEdx, double sigma, double x0, double y0, double z0)
@@ -548,6 +648,23 @@ int mfo_set_jet_source(mfo_ctx* c, double dEdx, double sigma, double x0, double 
     if (!c) return MFO_EINVAL;
     if (dEdx != 0.0 && !(sigma > 0.0)) return fail(c, MFO_EINVAL, "sigma must be > 0");
     c->jet_dEdx = dEdx; c->jet_sigma = sigma > 0.0 ? sigma : 1.0; c->jet_x0[0] = x0; c->jet_x0[1] = y0; c->jet_x0[2] = z0;
+    return MFO_OK;
+}
+int mfo_set_eos_table(mfo_ctx* c, int ne, int nn, double ln_e0, double dln_e, double n0, double dn, const double* ln_p)
+{
+    if (!c) return MFO_EINVAL;
+    if (c->eos != MFO_EOS_TABLE) return fail(c, MFO_EINVAL, "context was not created with MFO_EOS_TABLE");
+    if (ne < 2 || nn < 1 || !(dln_e > 0.0) || (nn > 1 && !(dn > 0.0)) || !ln_p) return fail(c, MFO_EINVAL, "bad table");
+    c->table.assign(ln_p, ln_p + (long)ne * nn);
+    c->P.kind = 1; c->P.ne = ne; c->P.nn = nn; c->P.ln_e0 = ln_e0; c->P.dln_e = dln_e; c->P.n0 = n0; c->P.dn = nn > 1 ? dn : 1.0;
+    c->P.lnp = c->table.data();
+    return MFO_OK;
+}
+int mfo_eos(mfo_ctx* c, double e, double n, double out[3])
+{
+    if (!c || !out) return MFO_EINVAL;
+    EosValue q = eos_eval(c->P, e, n);
+    out[0] = q.p; out[1] = q.p_e; out[2] = q.p_n;
     return MFO_OK;
 }
 int mfo_sync(mfo_ctx* c) { return c ? c->status : MFO_EINVAL; }
@@ -558,14 +675,14 @@ double mfo_slope(int limiter, double a, double b) { return slope2(limiter, a, b)
 int mfo_flux(mfo_ctx* c, int d, const double U[5], double F[5])
 {
     if (!c || !U || !F || d < 0 || d > 2) return MFO_EINVAL;
-    flux_d(c->cs2, d, U, F);
+    flux_d(c->P, d, U, F);
     return MFO_OK;
 }
 
 int mfo_musta_flux(mfo_ctx* c, int d, double lam, const double UL[5], const double UR[5], double F[5])
 {
     if (!c || !UL || !UR || !F || d < 0 || d > 2 || !(lam > 0.0)) return MFO_EINVAL;
-    musta_flux(c->cs2, d, c->k, lam, 0.5 * c->alpha * lam, 0.5 / (c->alpha * lam), UL, UR, F);
+    musta_flux(c->P, d, c->k, lam, 0.5 * c->alpha * lam, 0.5 / (c->alpha * lam), UL, UR, F);
     return MFO_OK;
 }
 

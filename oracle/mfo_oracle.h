@@ -47,6 +47,9 @@ int mfo_set_cs2(mfo_ctx*, double cs2);
 int mfo_set_predictor(mfo_ctx*, int on);
 int mfo_set_alpha(mfo_ctx*, double alpha);
 int mfo_set_jet_source(mfo_ctx*, double dEdx, double sigma, double x0, double y0, double z0);
+/* tabulated EOS (context created with MFO_EOS_TABLE): ln p on a grid uniform in ln e (ne points) and in n (nn points, e fastest) */
+int mfo_set_eos_table(mfo_ctx*, int ne, int nn, double ln_e0, double dln_e, double n0, double dn, const double* ln_p);
+int mfo_eos(mfo_ctx*, double e, double n, double out[3]);   /* p, dp/de, dp/dn of the context's EOS */
 int mfo_sync(mfo_ctx*);
 const char* mfo_last_error(mfo_ctx*);
 

@@ -116,6 +116,32 @@ def jet_event(n=512, dx=0.04, shape=None):
     return st
 
 
+def eos_table_from(p_of_e_n, e_min=1e-4, e_max=1e3, ne=257, n_max=12.0, nn=25):
+    """Tabulate an equation of state p(e, n) the way the library wants it: ln p on a grid uniform in ln e and uniform in n
+    (shape (nn, ne), e fastest).  nn = 1 gives a table without n dependence.  Pure data: the method's arithmetic is not here."""
+    ln_e = np.linspace(math.log(e_min), math.log(e_max), ne)
+    n = np.linspace(0.0, n_max, nn) if nn > 1 else np.zeros(1)
+    e2, n2 = np.meshgrid(np.exp(ln_e), n, indexing="xy")               # (nn, ne)
+    ln_p = np.log(p_of_e_n(e2, n2))
+    return dict(ln_e0=float(ln_e[0]), dln_e=float(ln_e[1] - ln_e[0]), n0=0.0, dn=float(n[1] - n[0]) if nn > 1 else 1.0,
+                ln_p=np.ascontiguousarray(ln_p))
+
+
+def linear_eos_table(cs2=1.0 / 3.0, nn=1, **kw):
+    """p = cs2*e as a table: ln p is linear in ln e, so the interpolation is exact and the run must reproduce the closed form."""
+    return eos_table_from(lambda e, n: cs2 * e + 0.0 * n, nn=nn, **kw)
+
+
+def crossover_eos_table(**kw):
+    """A smooth synthetic crossover EOS of our own making (no lattice table is available offline): p/e rises from ~0.22 to 1/3
+    around e ~ 2 and carries a mild charge dependence.  0 < dp/de < 1 everywhere."""
+    def p(e, n):
+        soft = 1.0 - 0.35 / (1.0 + (e / 2.0) ** 1.5)
+        charge = 1.0 + 0.08 * n * n / ((1.0 + n * n) * (1.0 + e))
+        return e / 3.0 * soft * charge
+    return eos_table_from(p, **kw)
+
+
 def config(index, scale=None):
     """BASELINE.json config `index` (1-based).  `scale` = (nz, ny, nx) replaces the grid, same dx, for parity sizes."""
     if index == 1:
