@@ -242,7 +242,8 @@ def run_ours(args):
 
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
-        g = MustaForce(nx, ny, nz, dx=st["dx"], path=args.path, stream=stream.cuda_stream, **sch)
+        eos_table = workloads.crossover_eos_table() if args.eos == "table" else None     # 8(f) row 1; not the metric's workload
+        g = MustaForce(nx, ny, nz, dx=st["dx"], path=args.path, stream=stream.cuda_stream, eos_table=eos_table, **sch)
         if "jet" in st:
             j = st["jet"]
             g.set_jet_source(j["dEdx"], j["sigma"], j["x0"], j["y0"], j["z0"])
@@ -337,7 +338,8 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "config": describe(st, {"path": g.path(), "l2": "state registers (%.0f MB each) exceed the 126 MB L2" % (40e-6 * cells)
                                     if 40 * cells > 126e6 else "state fits in L2 (small grid)", "parallelism": "replicas x%d" % world,
-                                    "status": status}),
+                                    "status": status, "eos": "p = e/3 (closed-form con2prim)" if args.eos == "cs2" else
+                                    "tabulated crossover p(e,n), Newton con2prim (roofline fractions below use the closed-form slot count)"}),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 40 * cells, "d2h_bytes_per_step": 40 * cells,
                     "steps": e2e_steps, "note": "mf_set_state(host) + mf_step(1) + mf_get_state(host) per step, pinned host buffers"},
@@ -364,6 +366,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (default 3 = the 256^3 metric workload)")
     ap.add_argument("--grid", default=None, help="nz,ny,nx override (parity/debug sizes)")
     ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid"])
+    ap.add_argument("--eos", default="cs2", choices=["cs2", "table"], help="table: synthetic crossover p(e,n) table with Newton con2prim")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--ref-crop", type=int, default=64, help="edge of the centred crop the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")

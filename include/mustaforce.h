@@ -37,7 +37,8 @@ extern "C" {
 
 typedef struct mf_ctx mf_ctx;
 
-enum { MF_EOS_CS2 = 0 /* p = cs2*e, default cs2 = 1/3 */ };
+enum { MF_EOS_CS2 = 0   /* p = cs2*e, default cs2 = 1/3: closed-form con2prim */,
+       MF_EOS_TABLE = 1 /* tabulated p(e, n) (Eq.2 :47) with Newton con2prim (Eq.23 :221-236); set with mf_set_eos_table */ };
 enum { MF_LIM_NONE = 0      /* Eq.14 central slope            :177 */,
        MF_LIM_MINMOD = 1    /* Minbee, Eq.18                  :201 */,
        MF_LIM_SUPERBEE = 2  /* Eq.19                          :203 */,
@@ -86,6 +87,12 @@ int mf_max_signal_speed(mf_ctx*, double* smax);
 int mf_set_rk(mf_ctx*, int order);          /* 2 (Eq.6, default) or 3 (Eq.7) */
 int mf_set_boundary(mf_ctx*, int bc);       /* MF_BC_OUTFLOW (default) or MF_BC_PERIODIC */
 int mf_set_cs2(mf_ctx*, double cs2);        /* 0 < cs2 < 1, default 1/3 */
+/* Tabulated equation of state for a context created with MF_EOS_TABLE (until it is set the context uses p = cs2*e).  ln_p is a HOST
+ * array of nn rows of ne values (e fastest): ln p at e = exp(ln_e0 + i*dln_e), n = n0 + j*dn.  Lookup: bilinear in (ln e, n) of ln p;
+ * the end cells extrapolate linearly in ln e, outside the n range the value is held; nn = 1: no n dependence.  con2prim then solves
+ * v (E + p(E - |M|v, R sqrt(1-v^2))) = |M| for the speed by safeguarded Newton (reading A18), and the CFL reduction uses the
+ * table's adiabatic sound speed.  The table is copied to the device; the call synchronises. */
+int mf_set_eos_table(mf_ctx*, int ne, int nn, double ln_e0, double dln_e, double n0, double dn, const double* ln_p);
 int mf_set_predictor(mf_ctx*, int on);      /* Eq.13 half step on (default, paper-literal) or off (MUSCL + RK) */
 int mf_set_alpha(mf_ctx*, double alpha);    /* FORCE alpha, default = number of active axes (:151) */
 /* Moving Gaussian energy-momentum source S_E = S_Mx = dEdx * G_sigma(x - (x0+t, y0, z0)) added to L in every RK

@@ -12,7 +12,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
 MF_OK, MF_EINVAL, MF_ENOMEM, MF_ECUDA, MF_ESTATE = 0, -1, -2, -3, -4
-MF_EOS_CS2 = 0
+MF_EOS_CS2, MF_EOS_TABLE = 0, 1
 LIM = {"none": 0, "minmod": 1, "superbee": 2, "vanalbada": 3, "vanleer": 4, "mc": 5, "first": 6}
 BC = {"outflow": 0, "periodic": 1}
 PATH = {"auto": 0, "staged": 1, "fused": 2, "hybrid": 3}
@@ -40,6 +40,7 @@ SIGNATURES = {
     "mf_set_rk": (C.c_int, [_vp, C.c_int]),
     "mf_set_boundary": (C.c_int, [_vp, C.c_int]),
     "mf_set_cs2": (C.c_int, [_vp, C.c_double]),
+    "mf_set_eos_table": (C.c_int, [_vp, C.c_int, C.c_int] + [C.c_double] * 4 + [_dp]),
     "mf_set_predictor": (C.c_int, [_vp, C.c_int]),
     "mf_set_alpha": (C.c_int, [_vp, C.c_double]),
     "mf_set_jet_source": (C.c_int, [_vp] + [C.c_double] * 5),
@@ -107,12 +108,12 @@ class MustaForce:
     """One mf_ctx.  Host arrays are numpy float64, shape (nz, ny, nx) or flat, x fastest."""
 
     def __init__(self, nx, ny=1, nz=1, dx=1.0, limiter="minmod", k_stages=2, rk=2, bc="outflow", predictor=True,
-                 alpha=None, cs2=None, path="auto", stream=None, strict=False):
+                 alpha=None, cs2=None, path="auto", stream=None, strict=False, eos_table=None):
         self.lib = load(strict)
         self.shape = (nz, ny, nx)
         self.n = nx * ny * nz
         lim = LIM[limiter] if isinstance(limiter, str) else int(limiter)
-        self.h = self.lib.mf_create(nx, ny, nz, float(dx), MF_EOS_CS2, lim, int(k_stages))
+        self.h = self.lib.mf_create(nx, ny, nz, float(dx), MF_EOS_CS2 if eos_table is None else MF_EOS_TABLE, lim, int(k_stages))
         if not self.h:
             raise MustaForceError(MF_EINVAL, self.lib.mf_last_error(None).decode())
         self._chk(self.lib.mf_set_rk(self.h, int(rk)))
@@ -125,6 +126,8 @@ class MustaForce:
         self._chk(self.lib.mf_set_path(self.h, PATH[path] if isinstance(path, str) else int(path)))
         if stream is not None:
             self.set_stream(stream)
+        if eos_table is not None:
+            self.set_eos_table(eos_table)
 
     def _chk(self, rc, allow=()):
         if rc != MF_OK and rc not in allow:
@@ -198,6 +201,13 @@ class MustaForce:
     # ---- options
     def set_jet_source(self, dEdx, sigma, x0, y0, z0):
         self._chk(self.lib.mf_set_jet_source(self.h, dEdx, sigma, x0, y0, z0))
+
+    def set_eos_table(self, tb):
+        """tb: dict(ln_e0, dln_e, n0, dn, ln_p) with ln_p of shape (nn, ne), e.g. workloads.crossover_eos_table()."""
+        ln_p = np.ascontiguousarray(tb["ln_p"], dtype=np.float64)
+        nn, ne = (1, ln_p.size) if ln_p.ndim == 1 else ln_p.shape
+        self._chk(self.lib.mf_set_eos_table(self.h, ne, nn, float(tb["ln_e0"]), float(tb["dln_e"]), float(tb.get("n0", 0.0)),
+                                            float(tb.get("dn", 1.0)), _p(ln_p)))
 
     def set_stream(self, stream):
         """stream: a raw cudaStream_t as int (e.g. torch.cuda.current_stream().cuda_stream); 0/None = own stream."""

@@ -33,6 +33,8 @@ struct mf_ctx {
     double* faces;           // staged path: 2*5*nact*next doubles
     double* fluxes;          // staged path: 5*nact*next doubles
     double* delta;           // fused path: Hancock increment, 5*next doubles
+    int eos;                 // MF_EOS_*
+    double* table;           // tabulated EOS: ln p, device copy
     int smax_valid;          // the device-side S_max accumulator already holds the reduction of the current U^n (fused into the last combine)
     StepState* ds;
     StepState* h_ds;         // pinned mirror
@@ -98,9 +100,17 @@ void set_eos(Eos& q, double cs2)
     q.vcap2 = V_CAP * V_CAP;
 }
 
+void clear_table(Eos& q)
+{
+    q.kind = 0; q.ne = q.nn = 0; q.pad = 0; q.ln_e0 = q.dln_e = q.n0 = q.dn = 0.0; q.lnp = nullptr;
+}
+
 int resolve_path(mf_ctx* c)
 {
-    if (c->path_req == MF_PATH_FUSED || c->path_req == MF_PATH_HYBRID) { if (!fused_supported(c->g)) return MF_EINVAL; c->path = c->path_req; }
+    if (c->path_req == MF_PATH_FUSED || c->path_req == MF_PATH_HYBRID) {
+        if (!fused_supported(c->g) || c->eos != MF_EOS_CS2) return MF_EINVAL;      // the tile kernel is built for p = cs2*e and three active axes
+        c->path = c->path_req;
+    }
     else if (c->path_req == MF_PATH_STAGED) c->path = MF_PATH_STAGED;
     else c->path = MF_PATH_STAGED;      // measured faster than the fused path on B200 so far (profiles/)
     return MF_OK;
@@ -253,7 +263,7 @@ mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k
     for (int a = 0; a < 3; ++a)
         if (n[a] < 1 || (n[a] > 1 && n[a] < 4)) { fail(nullptr, MF_EINVAL, "each extent must be 1 (inactive) or >= 4"); return nullptr; }
     if (!(dx > 0.0)) { fail(nullptr, MF_EINVAL, "dx must be > 0"); return nullptr; }
-    if (eos != MF_EOS_CS2) { fail(nullptr, MF_EINVAL, "unknown eos"); return nullptr; }
+    if (eos != MF_EOS_CS2 && eos != MF_EOS_TABLE) { fail(nullptr, MF_EINVAL, "unknown eos"); return nullptr; }
     if (limiter < 0 || limiter > MF_LIM_FIRST) { fail(nullptr, MF_EINVAL, "unknown limiter"); return nullptr; }
     if (k_stages < 0 || k_stages > 8) { fail(nullptr, MF_EINVAL, "k_stages must be in 0..8"); return nullptr; }
 
@@ -291,6 +301,8 @@ mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k
     g.es[0] = 1; g.es[1] = g.e[0]; g.es[2] = (long long)g.e[0] * g.e[1];
     g.dx = dx;
     set_eos(c->q, 1.0 / 3.0);
+    clear_table(c->q);
+    c->eos = eos; c->table = nullptr;
     c->limiter = limiter; c->k = k_stages; c->rk = 2; c->predictor = 1;
     c->alpha = c->nact > 0 ? (double)c->nact : 1.0;                 // A9
     memset(&c->src, 0, sizeof(c->src));
@@ -328,6 +340,7 @@ void mf_destroy(mf_ctx* c)
     if (c->faces) cudaFree(c->faces);
     if (c->fluxes) cudaFree(c->fluxes);
     if (c->delta) cudaFree(c->delta);
+    if (c->table) cudaFree(c->table);
     if (c->ds) cudaFree(c->ds);
     if (c->h_ds) cudaFreeHost(c->h_ds);
     if (c->partials) cudaFree(c->partials);
@@ -600,6 +613,21 @@ int mf_set_cs2(mf_ctx* c, double cs2)
     if (!(cs2 > 0.0) || !(cs2 < 1.0)) return fail(c, MF_EINVAL, "cs2 must be in (0,1)");
     set_eos(c->q, cs2); return MF_OK;
 }
+int mf_set_eos_table(mf_ctx* c, int ne, int nn, double ln_e0, double dln_e, double n0, double dn, const double* ln_p)
+{
+    if (!c) return MF_EINVAL;
+    if (c->eos != MF_EOS_TABLE) return fail(c, MF_EINVAL, "context was not created with MF_EOS_TABLE");
+    if (ne < 2 || nn < 1 || !(dln_e > 0.0) || (nn > 1 && !(dn > 0.0)) || !ln_p) return fail(c, MF_EINVAL, "bad table");
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->table) { cudaFree(c->table); c->table = nullptr; }
+    const size_t bytes = sizeof(double) * (size_t)ne * nn;
+    if (cudaMalloc(&c->table, bytes) != cudaSuccess) { cudaGetLastError(); c->table = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(EOS table) failed"); }
+    MF_CUDA(c, cudaMemcpy(c->table, ln_p, bytes, cudaMemcpyHostToDevice));
+    c->q.kind = 1; c->q.ne = ne; c->q.nn = nn; c->q.ln_e0 = ln_e0; c->q.dln_e = dln_e; c->q.n0 = n0; c->q.dn = nn > 1 ? dn : 1.0;
+    c->q.lnp = c->table;
+    c->smax_valid = 0;
+    return MF_OK;
+}
 int mf_set_predictor(mf_ctx* c, int on) { if (!c) return MF_EINVAL; c->predictor = on ? 1 : 0; return MF_OK; }
 int mf_set_alpha(mf_ctx* c, double alpha)
 {
@@ -626,7 +654,7 @@ int mf_set_path(mf_ctx* c, int path)
     if (path < MF_PATH_AUTO || path > MF_PATH_HYBRID) return fail(c, MF_EINVAL, "unknown path");
     int keep = c->path_req;
     c->path_req = path;
-    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "the fused path does not support this configuration (it needs three active axes)"); }
+    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "the fused path does not support this configuration (it needs three active axes and MF_EOS_CS2)"); }
     return MF_OK;
 }
 int mf_get_path(mf_ctx* c, int* path) { if (!c || !path) return MF_EINVAL; *path = c->path; return MF_OK; }

@@ -22,7 +22,99 @@ struct Eos {
     double qc1sq;   // c1*c1/4
     double hc1;     // c1/2
     double vcap2;   // V_CAP^2
+    // tabulated EOS (kind 1, reading A18): ln p on a grid uniform in ln e (ne points) and in n (nn points), e fastest, device memory
+    int kind, ne, nn, pad;
+    double ln_e0, dln_e, n0, dn;
+    const double* lnp;
 };
+
+struct EosValue {
+    double p, p_e, p_n;   // p, dp/de at fixed n, dp/dn at fixed e
+};
+
+// The table part of the EOS lives in NON-inlined device functions that take the table by value, so that the p = cs2*e kernels keep their
+// register allocation: all they carry is a predicate on q.kind and a call on the cold path.
+struct TableRef {
+    const double* lnp;
+    int ne, nn;
+    double ln_e0, dln_e, n0, dn;
+};
+__device__ __forceinline__ TableRef table_of(const Eos& q)
+{
+    TableRef t; t.lnp = q.lnp; t.ne = q.ne; t.nn = q.nn; t.ln_e0 = q.ln_e0; t.dln_e = q.dln_e; t.n0 = q.n0; t.dn = q.dn;
+    return t;
+}
+
+// Eq.2 :47, p = p(e, n) from the table: bilinear interpolation of ln p in (ln e, n); the end cells extrapolate linearly in (ln e, ln p),
+// outside the n range the value is held.
+static __device__ __noinline__ EosValue eos_table_eval(TableRef q, double e, double n)
+{
+    EosValue r;
+    const double x = (log(e) - q.ln_e0) / q.dln_e;
+    int i = (int)floor(x);
+    i = max(0, min(i, q.ne - 2));
+    const double fx = x - (double)i;
+    int j = 0;
+    double fy = 0.0;
+    bool n_inside = false;
+    if (q.nn > 1) {
+        const double y = (n - q.n0) / q.dn;
+        j = (int)floor(y);
+        j = max(0, min(j, q.nn - 2));
+        fy = y - (double)j;
+        n_inside = fy >= 0.0 && fy <= 1.0;
+        fy = fmin(fmax(fy, 0.0), 1.0);
+    }
+    const double* row0 = q.lnp + (long long)j * q.ne;
+    const double* row1 = q.nn > 1 ? row0 + q.ne : row0;
+    const double d0 = __ldg(row0 + i + 1) - __ldg(row0 + i), d1 = __ldg(row1 + i + 1) - __ldg(row1 + i);
+    const double l0 = __ldg(row0 + i) + fx * d0, l1 = __ldg(row1 + i) + fx * d1;
+    const double lp = l0 + fy * (l1 - l0);
+    r.p = exp(lp);
+    const double dlnp_dlne = ((1.0 - fy) * d0 + fy * d1) / q.dln_e;
+    r.p_e = r.p * dlnp_dlne / e;
+    r.p_n = n_inside ? r.p * ((l1 - l0) / q.dn) : 0.0;
+    return r;
+}
+
+// EK is a COMPILE-TIME switch (0: p = cs2*e, 1: table): the kernels are instantiated twice and the launchers pick by q.kind, so that
+// the closed-form instantiations do not carry a single instruction or register of the table path.
+template <int EK = 0>
+__device__ __forceinline__ EosValue eos_eval(const Eos& q, double e, double n)
+{
+    if (EK == 0) { EosValue r; r.p = q.cs2 * e; r.p_e = q.cs2; r.p_n = 0.0; return r; }
+    return eos_table_eval(table_of(q), e, n);
+}
+
+// Eq.23 :231-236 for a tabulated p(e, n): Newton on f(v) = v (E + p(E - |M| v, R sqrt(1 - v^2))) - |M| from v = |M|/E, bisection whenever
+// a step leaves the bracket, at most 60 iterations, stop at |dv| <= 1e-15.  Data-dependent trip count: lanes of a warp wait for the
+// slowest.  out = (speed, e, p).
+struct SpeedEP {
+    double v, e, p;
+};
+static __device__ __noinline__ SpeedEP solve_speed(TableRef q, double E, double M, double R)
+{
+    double lo = 0.0, hi = M / E, v = hi;
+    for (int it = 0; it < 60; ++it) {
+        const double e = E - M * v;
+        const double g = sqrt(1.0 - v * v);
+        const EosValue w = eos_table_eval(q, e, R * g);
+        const double f = v * (E + w.p) - M;
+        if (f == 0.0) break;
+        if (f > 0.0) hi = v; else lo = v;
+        const double df = E + w.p + v * (-M * w.p_e - R * (v / g) * w.p_n);
+        double vn = v - f / df;
+        if (!(vn > lo && vn < hi)) vn = 0.5 * (lo + hi);
+        const double dv = fabs(vn - v);
+        v = vn;
+        if (dv <= 1e-15) break;
+    }
+    SpeedEP r;
+    r.v = v;
+    r.e = E - M * v;
+    r.p = eos_table_eval(q, r.e, R * sqrt(1.0 - v * v)).p;
+    return r;
+}
 
 // ---- Eq.14-21 in two-argument form (A6): a = U_i - U_{i-1}, b = U_{i+1} - U_i; returns the limited slope
 template <int LIM>
@@ -78,7 +170,8 @@ __device__ __forceinline__ double sqrt_pos(double x)          // sqrt(x) for nor
 
 // ---- Eq.23 for p = cs2*e in closed form with the admissibility guard A12.  :227-234
 // Returns the three velocity components and the pressure.
-__device__ __forceinline__ void velocity_pressure(const Eos& q, double E, double Mx, double My, double Mz,
+template <int EK = 0>
+__device__ __forceinline__ void velocity_pressure(const Eos& q, double E, double Mx, double My, double Mz, double R,
                                                   double& vx, double& vy, double& vz, double& e, double& p)
 {
     double M2 = Mx * Mx + My * My + Mz * Mz;
@@ -93,6 +186,14 @@ __device__ __forceinline__ void velocity_pressure(const Eos& q, double E, double
         Mx *= s; My *= s; Mz *= s;
         M2 = Mx * Mx + My * My + Mz * Mz;
     }
+    if (EK != 0) {                                // tabulated EOS: Newton on the speed, then v_j = M_j v/|M|
+        const double M = sqrt(M2);
+        if (M == 0.0) { vx = vy = vz = 0.0; e = E; p = eos_table_eval(table_of(q), E, R).p; return; }
+        const SpeedEP r = solve_speed(table_of(q), E, M, R);
+        const double s = r.v / M;
+        vx = Mx * s; vy = My * s; vz = Mz * s; e = r.e; p = r.p;
+        return;
+    }
     double Q = sqrt_pos(q.c1sq * E * E - q.four_cs2 * M2);
     double inv = two_over(q.c1 * E + Q);
     vx = Mx * inv; vy = My * inv; vz = Mz * inv;
@@ -105,11 +206,11 @@ __device__ __forceinline__ void velocity_pressure(const Eos& q, double E, double
 }
 
 // ---- Eq.3 :53-59: F_d(U) = ((E+p)v_d, M_j v_d + p delta_jd, R v_d)
-template <int D>
+template <int D, int EK = 0>
 __device__ __forceinline__ void flux_d(const Eos& q, const double (&U)[5], double (&F)[5])
 {
     double vx, vy, vz, e, p;
-    velocity_pressure(q, U[0], U[1], U[2], U[3], vx, vy, vz, e, p);
+    velocity_pressure<EK>(q, U[0], U[1], U[2], U[3], U[4], vx, vy, vz, e, p);
     double vd = D == 0 ? vx : (D == 1 ? vy : vz);
     F[0] = (U[0] + p) * vd;
     F[1] = U[1] * vd;
@@ -153,44 +254,26 @@ __device__ __forceinline__ bool flux_fast(const Eos& q, const double (&U)[5], do
 #endif
 
 // flux evaluation used outside MUSTA (Hancock predictor): fast path with the guarded fallback
-template <int D>
+template <int D, int EK = 0>
 __device__ __forceinline__ void flux_eval(const Eos& q, const double (&U)[5], double (&F)[5])
 {
 #ifdef MF_STRICT
-    flux_d<D>(q, U, F);
+    flux_d<D, EK>(q, U, F);
 #else
+    if (EK != 0) { flux_d<D, EK>(q, U, F); return; }
     if (!flux_fast<D>(q, U, F)) flux_d<D>(q, U, F);
 #endif
 }
 
 // ---- MUSTA_k with FORCE-alpha, steps 1-5 :123-135, Eq.8-11 :130-149 (A1: Richtmyer state uses the flux difference)
 // A, B are U_L^(0), U_R^(0) on entry and are overwritten.
-template <int D>
+template <int D, int EK = 0>
 __device__ __forceinline__ void musta_flux(const Eos& q, int k, double lam, double c_lw, double c_lf,
                                            double (&A)[5], double (&B)[5], double (&F)[5])
 {
-#ifdef MF_STRICT
-    for (int l = 0;; ++l) {
-        double FA[5], FB[5], W[5];
-        flux_d<D>(q, A, FA);
-        flux_d<D>(q, B, FB);
-#pragma unroll
-        for (int c = 0; c < 5; ++c) W[c] = 0.5 * (A[c] + B[c]) - c_lw * (FB[c] - FA[c]);      // Eq.10
-        flux_d<D>(q, W, F);                                                                   // F^lw
-#pragma unroll
-        for (int c = 0; c < 5; ++c) {
-            double Flf = 0.5 * (FA[c] + FB[c]) - c_lf * (B[c] - A[c]);                        // Eq.11
-            F[c] = 0.5 * (F[c] + Flf);                                                        // Eq.9
-        }
-        if (l == k) break;
-#pragma unroll
-        for (int c = 0; c < 5; ++c) {                                                         // Eq.8
-            A[c] = A[c] - lam * (F[c] - FA[c]);
-            B[c] = B[c] - lam * (FB[c] - F[c]);
-        }
-    }
-#else
-    // same formulas with the constant factors folded so that every line is one FP64 instruction
+#ifndef MF_STRICT
+    if (EK == 0) {
+    // the formulas below with the constant factors folded so that every line is one FP64 instruction, and the 26-instruction flux
     const double hc_lf = 0.5 * c_lf;
     for (int l = 0;; ++l) {
         double FA[5], FB[5], W[5];
@@ -210,19 +293,51 @@ __device__ __forceinline__ void musta_flux(const Eos& q, int k, double lam, doub
             B[c] = fma(-lam, FB[c] - F[c], B[c]);
         }
     }
+    return;
+    }
 #endif
+    for (int l = 0;; ++l) {
+        double FA[5], FB[5], W[5];
+        flux_d<D, EK>(q, A, FA);
+        flux_d<D, EK>(q, B, FB);
+#pragma unroll
+        for (int c = 0; c < 5; ++c) W[c] = 0.5 * (A[c] + B[c]) - c_lw * (FB[c] - FA[c]);      // Eq.10
+        flux_d<D, EK>(q, W, F);                                                               // F^lw
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+            double Flf = 0.5 * (FA[c] + FB[c]) - c_lf * (B[c] - A[c]);                        // Eq.11
+            F[c] = 0.5 * (F[c] + Flf);                                                        // Eq.9
+        }
+        if (l == k) break;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {                                                         // Eq.8
+            A[c] = A[c] - lam * (F[c] - FA[c]);
+            B[c] = B[c] - lam * (FB[c] - F[c]);
+        }
+    }
 }
 
 // ---- a2: local signal speed (|v|+cs)/(1+|v|cs) (A10) and the state check behind MF_ESTATE
+template <int EK = 0>
 __device__ __forceinline__ double signal_speed(const Eos& q, double E, double Mx, double My, double Mz, double R, int& bad)
 {
     bool finite = isfinite(E) && isfinite(Mx) && isfinite(My) && isfinite(Mz) && isfinite(R);
     if (!finite) { bad = 1; return 0.0; }
     if (E > E_VACUUM && Mx * Mx + My * My + Mz * Mz > E * E) bad = 1;
     double vx, vy, vz, e, p;
-    velocity_pressure(q, E, Mx, My, Mz, vx, vy, vz, e, p);
+    velocity_pressure<EK>(q, E, Mx, My, Mz, R, vx, vy, vz, e, p);
     double av = sqrt(vx * vx + vy * vy + vz * vz);
-    return (av + q.cs) / (1.0 + av * q.cs);
+    double cs = q.cs;
+    if (EK != 0) {                            // adiabatic sound speed of the table: cs^2 = p_e + n p_n/(e+p)
+        double cs2t = 0.0;
+        if (e > 0.0) {
+            const double nn = R * sqrt(1.0 - av * av);
+            const EosValue w = eos_table_eval(table_of(q), e, nn);
+            cs2t = w.p_e + nn * w.p_n / (e + w.p);
+        }
+        cs = cs2t > 0.0 ? sqrt(cs2t) : 0.0;
+    }
+    return (av + cs) / (1.0 + av * cs);
 }
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }

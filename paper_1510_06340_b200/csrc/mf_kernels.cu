@@ -46,13 +46,14 @@ __device__ __forceinline__ void block_reduce_smax(double smax, int bad, StepStat
     }
 }
 
+template <int EK>
 __global__ void __launch_bounds__(TPB) k_cfl(Grid g, Eos q, CState5 U, StepState* ds)
 {
     double smax = 0.0;
     int bad = 0;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < g.ncell; o += stride) {
-        double s = signal_speed(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], U.q[4][o], bad);
+        double s = signal_speed<EK>(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], U.q[4][o], bad);
         smax = fmax(smax, s);
     }
     block_reduce_smax(smax, bad, ds);
@@ -63,7 +64,7 @@ int launch_cfl(const Grid& g, const Eos& q, CState5 U, StepState* ds, int num_sm
     unsigned int nb = blocks_for(g.ncell, TPB);
     unsigned int cap = (unsigned int)num_sms * 8u;
     if (nb > cap) nb = cap;
-    k_cfl<<<nb, TPB, 0, st>>>(g, q, U, ds);
+    if (q.kind) k_cfl<1><<<nb, TPB, 0, st>>>(g, q, U, ds); else k_cfl<0><<<nb, TPB, 0, st>>>(g, q, U, ds);
     return 1;
 }
 
@@ -108,7 +109,7 @@ int launch_reset(StepState* ds, cudaStream_t st) { k_reset<<<1, 1, 0, st>>>(ds);
 
 // =========================================================================== a3 + a4: cell stage
 // One thread per cell of the extended region (interior + 1 layer on every active axis).
-template <int LIM>
+template <int LIM, int EK>
 __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, int predictor, CState5 V, Faces fc, const StepState* ds)
 {
     // linear index over the extended region, x fastest: 256 consecutive cells per block (measured on B200: 32 x 8 tiles, which
@@ -149,19 +150,19 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
         bool first = true;
         double Fl[5], Fr[5];
         if (g.act[0]) {
-            flux_eval<0>(q, UL[0], Fl); flux_eval<0>(q, UR[0], Fr);
+            flux_eval<0, EK>(q, UL[0], Fl); flux_eval<0, EK>(q, UR[0], Fr);
 #pragma unroll
             for (int v = 0; v < 5; ++v) delta[v] = hl * (Fl[v] - Fr[v]);
             first = false;
         }
         if (g.act[1]) {
-            flux_eval<1>(q, UL[1], Fl); flux_eval<1>(q, UR[1], Fr);
+            flux_eval<1, EK>(q, UL[1], Fl); flux_eval<1, EK>(q, UR[1], Fr);
 #pragma unroll
             for (int v = 0; v < 5; ++v) { double t = hl * (Fl[v] - Fr[v]); delta[v] = first ? t : delta[v] + t; }
             first = false;
         }
         if (g.act[2]) {
-            flux_eval<2>(q, UL[2], Fl); flux_eval<2>(q, UR[2], Fr);
+            flux_eval<2, EK>(q, UL[2], Fl); flux_eval<2, EK>(q, UR[2], Fr);
 #pragma unroll
             for (int v = 0; v < 5; ++v) { double t = hl * (Fl[v] - Fr[v]); delta[v] = first ? t : delta[v] + t; }
         }
@@ -215,21 +216,21 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
         if (g.act[0]) {
 #pragma unroll
             for (int v = 0; v < 5; ++v) { UL[v] = U0[v] - H[0][v]; UR[v] = U0[v] + H[0][v]; }
-            flux_eval<0>(q, UL, Fl); flux_eval<0>(q, UR, Fr);
+            flux_eval<0, EK>(q, UL, Fl); flux_eval<0, EK>(q, UR, Fr);
 #pragma unroll
             for (int v = 0; v < 5; ++v) acc[v] += Fl[v] - Fr[v];
         }
         if (g.act[1]) {
 #pragma unroll
             for (int v = 0; v < 5; ++v) { UL[v] = U0[v] - H[1][v]; UR[v] = U0[v] + H[1][v]; }
-            flux_eval<1>(q, UL, Fl); flux_eval<1>(q, UR, Fr);
+            flux_eval<1, EK>(q, UL, Fl); flux_eval<1, EK>(q, UR, Fr);
 #pragma unroll
             for (int v = 0; v < 5; ++v) acc[v] += Fl[v] - Fr[v];
         }
         if (g.act[2]) {
 #pragma unroll
             for (int v = 0; v < 5; ++v) { UL[v] = U0[v] - H[2][v]; UR[v] = U0[v] + H[2][v]; }
-            flux_eval<2>(q, UL, Fl); flux_eval<2>(q, UR, Fr);
+            flux_eval<2, EK>(q, UL, Fl); flux_eval<2, EK>(q, UR, Fr);
 #pragma unroll
             for (int v = 0; v < 5; ++v) acc[v] += Fl[v] - Fr[v];
         }
@@ -246,7 +247,8 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
 {
     const unsigned int nb = blocks_for(g.next, TPB);
     switch (limiter) {
-#define MF_CASE(L) case L: k_cell_stage<L><<<nb, TPB, 0, st>>>(g, q, predictor, V, fc, ds); break;
+#define MF_CASE(L) case L: if (q.kind) k_cell_stage<L, 1><<<nb, TPB, 0, st>>>(g, q, predictor, V, fc, ds); \
+                           else k_cell_stage<L, 0><<<nb, TPB, 0, st>>>(g, q, predictor, V, fc, ds); break;
         MF_CASE(LIM_NONE) MF_CASE(LIM_MINMOD) MF_CASE(LIM_SUPERBEE) MF_CASE(LIM_VANALBADA) MF_CASE(LIM_VANLEER) MF_CASE(LIM_MC) MF_CASE(LIM_FIRST)
 #undef MF_CASE
     default: return 0;
@@ -256,7 +258,7 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
 
 // =========================================================================== a5 + a6: interface fluxes
 // One thread per interface between cell c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
-template <int D>
+template <int D, int EK>
 __global__ void __launch_bounds__(TPB, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, int k, Faces fc, Fluxes fx, const StepState* ds)
 {
     int m[3] = { g.n[0], g.n[1], g.n[2] };
@@ -283,7 +285,7 @@ __global__ void __launch_bounds__(TPB, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q,
         for (int v = 0; v < 5; ++v) { A[v] = fc.f[dW][1][v][p] + fc.f[D][0][v][p]; B[v] = fc.f[dW][1][v][pn] - fc.f[D][0][v][pn]; }
     }
 #endif
-    musta_flux<D>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
+    musta_flux<D, EK>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
 #pragma unroll
     for (int v = 0; v < 5; ++v) fx.f[D][v][p] = F[v];
 }
@@ -296,9 +298,9 @@ int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, F
         long long total = 1;
         for (int a = 0; a < 3; ++a) total *= (a == d) ? g.n[a] + 1 : g.n[a];
         unsigned int nb = blocks_for(total, TPB);
-        if (d == 0) k_flux_stage<0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds);
-        if (d == 1) k_flux_stage<1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds);
-        if (d == 2) k_flux_stage<2><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds);
+        if (d == 0) { if (q.kind) k_flux_stage<0, 1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<0, 0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); }
+        if (d == 1) { if (q.kind) k_flux_stage<1, 1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<1, 0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); }
+        if (d == 2) { if (q.kind) k_flux_stage<2, 1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<2, 0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); }
         ++launches;
     }
     return launches;
@@ -326,6 +328,7 @@ __device__ __forceinline__ double rk_form(const Stage& sg, double ua, double ub,
     return L;                                                      // form 3: L itself (mf_eval_L)
 }
 
+template <int EK>
 __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds)
 {
     const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -358,14 +361,15 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
             W[v] = rk_form(sg, ua, ub, dt, L);
             out.q[v][o] = W[v];
         }
-        if (sg.cfl) smax = signal_speed(q, W[0], W[1], W[2], W[3], W[4], bad);   // a2 for the next step, while U^{n+1} is in registers
+        if (sg.cfl) smax = signal_speed<EK>(q, W[0], W[1], W[2], W[3], W[4], bad);   // a2 for the next step, while U^{n+1} is in registers
     }
     if (sg.cfl) block_reduce_smax(smax, bad, ds);
 }
 
 int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds, cudaStream_t st)
 {
-    k_combine<<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+    if (q.kind) k_combine<1><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+    else k_combine<0><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
     return 1;
 }
 
@@ -378,6 +382,7 @@ int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua,
 // 64 registers / 4 blocks per SM: measured on B200, 32 resident warps let the combine's loads of one block overlap the MUSTA of the
 // others (1.37 ms per launch at 256^3 against 1.56 ms at 24 warps; prefetching the operands with cp.async into shared memory at 24
 // warps did not help, 1.53 ms: the kernel is then limited by DRAM bandwidth, not by latency).
+template <int EK>
 __global__ void __launch_bounds__(TPB, 4) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
                                                           Source src, StepState* ds)
 {
@@ -413,7 +418,7 @@ __global__ void __launch_bounds__(TPB, 4) k_xflux_combine(Grid g, Eos q, int k, 
                 if (sg.form == 1 || sg.form == 2) prefetch_l2(&Ub.q[v][o]);
             }
         }
-        musta_flux<0>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
+        musta_flux<0, EK>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
     }
 #pragma unroll
     for (int v = 0; v < 5; ++v) sF[v][t] = F[v];
@@ -439,7 +444,7 @@ __global__ void __launch_bounds__(TPB, 4) k_xflux_combine(Grid g, Eos q, int k, 
             W[v] = rk_form(sg, ua, ub, dt, L);
             out.q[v][o] = W[v];
         }
-        if (sg.cfl) smax = signal_speed(q, W[0], W[1], W[2], W[3], W[4], bad);
+        if (sg.cfl) smax = signal_speed<EK>(q, W[0], W[1], W[2], W[3], W[4], bad);
     }
     if (sg.cfl) block_reduce_smax(smax, bad, ds);
 }
@@ -448,40 +453,43 @@ int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx
                          StepState* ds, cudaStream_t st)
 {
     const long long total = (long long)(g.n[0] + 1) * g.n[1] * g.n[2];
-    k_xflux_combine<<<blocks_for(total, TPB - 1), TPB, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds);
+    if (q.kind) k_xflux_combine<1><<<blocks_for(total, TPB - 1), TPB, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds);
+    else k_xflux_combine<0><<<blocks_for(total, TPB - 1), TPB, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds);
     return 1;
 }
 
 // =========================================================================== conversions
+template <int EK>
 __global__ void __launch_bounds__(TPB) k_prim2con(Grid g, Eos q, State5 U)
 {
     const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= g.ncell) return;
     double e = U.q[0][o], vx = U.q[1][o], vy = U.q[2][o], vz = U.q[3][o], n = U.q[4][o];
-    double p = q.cs2 * e;                                          // Eq.4 :63-67
+    double p = eos_eval<EK>(q, e, n).p;                                // Eq.4 :63-67
     double g2 = 1.0 / (1.0 - (vx * vx + vy * vy + vz * vz));
     double w = (e + p) * g2;
     U.q[0][o] = w - p; U.q[1][o] = w * vx; U.q[2][o] = w * vy; U.q[3][o] = w * vz; U.q[4][o] = n * sqrt(g2);
 }
 
+template <int EK>
 __global__ void __launch_bounds__(TPB) k_con2prim(Grid g, Eos q, CState5 U, State5 P)
 {
     const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= g.ncell) return;
     double vx, vy, vz, e, p;
-    velocity_pressure(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], vx, vy, vz, e, p);
+    velocity_pressure<EK>(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], U.q[4][o], vx, vy, vz, e, p);
     P.q[0][o] = e; P.q[1][o] = vx; P.q[2][o] = vy; P.q[3][o] = vz;
     P.q[4][o] = U.q[4][o] * sqrt(1.0 - (vx * vx + vy * vy + vz * vz));   // n = R sqrt(1-v^2), Eq.23
 }
 
 int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st)
 {
-    k_prim2con<<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U);
+    if (q.kind) k_prim2con<1><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U); else k_prim2con<0><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U);
     return 1;
 }
 int launch_con2prim(const Grid& g, const Eos& q, CState5 U, State5 P, cudaStream_t st)
 {
-    k_con2prim<<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U, P);
+    if (q.kind) k_con2prim<1><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U, P); else k_con2prim<0><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U, P);
     return 1;
 }
 
