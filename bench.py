@@ -144,16 +144,18 @@ class ClockSampler:
 
 def make_workload(args):
     shape = tuple(int(x) for x in args.grid.split(",")) if args.grid else None
-    if args.config == 3 and shape is None:
-        return workloads.gaussian_hot_spot()
-    return workloads.config(args.config, scale=shape)
+    st = workloads.gaussian_hot_spot() if (args.config == 3 and shape is None) else workloads.config(args.config, scale=shape)
+    if args.predictor == "off":
+        st["scheme"] = dict(st["scheme"], predictor=False)
+    return st
 
 
 def describe(st, extra=None):
     nz, ny, nx = st["shape"]
     cfg = {"workload": "%s %dx%dx%d dx=%g %s k=%d RK%d %s cfl=%g" % (
         st["name"], nx, ny, nz, st["dx"], st["scheme"]["limiter"], st["scheme"]["k_stages"], st["scheme"]["rk"],
-        st["scheme"]["bc"], st["cfl"]), "cells": nx * ny * nz, "predictor": "on (paper-literal Eq.13)"}
+        st["scheme"]["bc"], st["cfl"]), "cells": nx * ny * nz,
+        "predictor": "on (paper-literal Eq.13)" if st["scheme"].get("predictor", True) else "off (MUSCL + RK, reading A4)"}
     if extra:
         cfg.update(extra)
     return cfg
@@ -301,10 +303,11 @@ def run_ours(args):
         return
 
     pk = peaks()
-    slots_cu, slots_L, slots_musta = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim)
+    pred_on = sch.get("predictor", True)
+    slots_cu, slots_L, slots_musta = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim, pred_on)
     alu_peak_slots = 148 * FP64_LANES_PER_SM * pk["sm_max_mhz"] * 1e6          # FP64 instructions/s, all SMs
     # dominant kernel, from the event pairs recorded around every launch inside the timed region
-    work = class_work(g.path(), sch["limiter"], sch["k_stages"], ndim, nx > 1)
+    work = class_work(g.path(), sch["limiter"], sch["k_stages"], ndim, nx > 1, pred_on)
     kernels = {}
     for name, (ms, groups) in prof.items():
         if name not in work or groups == 0:
@@ -367,6 +370,7 @@ def main():
     ap.add_argument("--grid", default=None, help="nz,ny,nx override (parity/debug sizes)")
     ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid"])
     ap.add_argument("--eos", default="cs2", choices=["cs2", "table"], help="table: synthetic crossover p(e,n) table with Newton con2prim")
+    ap.add_argument("--predictor", default="on", choices=["on", "off"], help="off: without the Hancock half step (reading A4), reported beside the default")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--ref-crop", type=int, default=64, help="edge of the centred crop the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
