@@ -382,8 +382,10 @@ int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua,
 // 64 registers / 4 blocks per SM: measured on B200, 32 resident warps let the combine's loads of one block overlap the MUSTA of the
 // others (1.37 ms per launch at 256^3 against 1.56 ms at 24 warps; prefetching the operands with cp.async into shared memory at 24
 // warps did not help, 1.53 ms: the kernel is then limited by DRAM bandwidth, not by latency).
-template <int EK>
-__global__ void __launch_bounds__(TPB, 4) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
+// FORM (the RK form of the stage) and CFL (last stage of a step) are compile-time: the stage loop has no form branches, and the
+// signal-speed code with its block reduction exists only in the instantiations that need it.
+template <int EK, int FORM, bool CFL>
+__global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
                                                           Source src, StepState* ds)
 {
     __shared__ double sF[5][TPB];
@@ -414,8 +416,8 @@ __global__ void __launch_bounds__(TPB, 4) k_xflux_combine(Grid g, Eos q, int k, 
             for (int v = 0; v < 5; ++v) {
                 if (g.act[1]) prefetch_l2(&fx.f[1][v][pc]);      // the neighbour lines (pc - es) are somebody else's pc: prefetching
                 if (g.act[2]) prefetch_l2(&fx.f[2][v][pc]);      // them too measured slower
-                if (sg.form != 3) prefetch_l2(&Ua.q[v][o]);
-                if (sg.form == 1 || sg.form == 2) prefetch_l2(&Ub.q[v][o]);
+                if (FORM != 3) prefetch_l2(&Ua.q[v][o]);
+                if (FORM == 1 || FORM == 2) prefetch_l2(&Ub.q[v][o]);
             }
         }
         musta_flux<0, EK>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
@@ -439,22 +441,30 @@ __global__ void __launch_bounds__(TPB, 4) k_xflux_combine(Grid g, Eos q, int k, 
             if (g.act[2]) acc = acc + (fx.f[2][v][pc] - fx.f[2][v][pc - g.es[2]]);
             double L = -acc / g.dx;                                        // Eq.1 :43
             if (src.on && v < 2) L = L + S;
-            double ua = sg.form == 3 ? 0.0 : Ua.q[v][o];
-            double ub = (sg.form == 1 || sg.form == 2) ? Ub.q[v][o] : 0.0;
-            W[v] = rk_form(sg, ua, ub, dt, L);
+            const double ua = FORM == 3 ? 0.0 : Ua.q[v][o];
+            const double ub = (FORM == 1 || FORM == 2) ? Ub.q[v][o] : 0.0;
+            W[v] = FORM == 0 ? ua + dt * L : (FORM == 1 ? 0.5 * (ua + ub + dt * L) : (FORM == 2 ? sg.ca * ua + sg.cb * ub + (sg.cdt * dt) * L : L));
             out.q[v][o] = W[v];
         }
-        if (sg.cfl) smax = signal_speed<EK>(q, W[0], W[1], W[2], W[3], W[4], bad);
+        if (CFL) smax = signal_speed<EK>(q, W[0], W[1], W[2], W[3], W[4], bad);
     }
-    if (sg.cfl) block_reduce_smax(smax, bad, ds);
+    if (CFL) block_reduce_smax(smax, bad, ds);
 }
 
 int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src,
                          StepState* ds, cudaStream_t st)
 {
     const long long total = (long long)(g.n[0] + 1) * g.n[1] * g.n[2];
-    if (q.kind) k_xflux_combine<1><<<blocks_for(total, TPB - 1), TPB, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds);
-    else k_xflux_combine<0><<<blocks_for(total, TPB - 1), TPB, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds);
+    const unsigned int nb = blocks_for(total, TPB - 1);
+#define MF_XFC(EK_, FORM_, CFL_) k_xflux_combine<EK_, FORM_, CFL_><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds)
+#define MF_XFC_FORMS(EK_) \
+    if (sg.form == 0) { if (sg.cfl) MF_XFC(EK_, 0, true); else MF_XFC(EK_, 0, false); } \
+    else if (sg.form == 1) { if (sg.cfl) MF_XFC(EK_, 1, true); else MF_XFC(EK_, 1, false); } \
+    else if (sg.form == 2) { if (sg.cfl) MF_XFC(EK_, 2, true); else MF_XFC(EK_, 2, false); } \
+    else MF_XFC(EK_, 3, false);
+    if (q.kind) { MF_XFC_FORMS(1) } else { MF_XFC_FORMS(0) }
+#undef MF_XFC_FORMS
+#undef MF_XFC
     return 1;
 }
 
