@@ -116,9 +116,8 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
     // reuse the y neighbours through L1, are 10-15% slower because the DRAM bursts get shorter)
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= g.next) return;
-    const int ie = (int)(p % g.e[0]);
-    const long long r = p / g.e[0];
-    const int je = (int)(r % g.e[1]), ke = (int)(r / g.e[1]);
+    int ie, je, ke;
+    unflatten3(p, g.e[0], g.e[1], g.idx32, ie, je, ke);
     const int c[3] = { ie - g.h[0], je - g.h[1], ke - g.h[2] };             // interior coordinates, may be -1 or n
     int cc[3];
 #pragma unroll
@@ -267,10 +266,7 @@ __global__ void __launch_bounds__(TPB, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q,
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= total) return;
     int c[3];
-    c[0] = (int)(t % m[0]);
-    long long r = t / m[0];
-    c[1] = (int)(r % m[1]);
-    c[2] = (int)(r / m[1]);
+    unflatten3(t, m[0], m[1], g.idx32, c[0], c[1], c[2]);
     c[D] -= 1;
     const long long p = (c[0] + g.h[0]) * g.es[0] + (c[1] + g.h[1]) * g.es[1] + (c[2] + g.h[2]) * g.es[2];
     double A[5], B[5], F[5];
@@ -335,9 +331,8 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
     double smax = 0.0;
     int bad = 0;
     if (o < g.ncell) {
-        const int i = (int)(o % g.n[0]);
-        const long long r = o / g.n[0];
-        const int j = (int)(r % g.n[1]), k = (int)(r / g.n[1]);
+        int i, j, k;
+        unflatten3(o, g.n[0], g.n[1], g.idx32, i, j, k);
         const long long p = (i + g.h[0]) * g.es[0] + (j + g.h[1]) * g.es[1] + (k + g.h[2]) * g.es[2];
         const double dt = ds->dt;
         double S = 0.0;
@@ -354,7 +349,11 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
                 acc = first ? diff : acc + diff;
                 first = false;
             }
+#ifdef MF_STRICT
             double L = -acc / g.dx;                                    // Eq.1 :43
+#else
+            double L = -acc * g.inv_dx;
+#endif
             if (src.on && v < 2) L = L + S;
             double ua = sg.form == 3 ? 0.0 : Ua.q[v][o];
             double ub = (sg.form == 1 || sg.form == 2) ? Ub.q[v][o] : 0.0;
@@ -398,9 +397,7 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
     long long p = 0;
     double F[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
     if (live) {
-        const long long r = I / nf;
-        f = (int)(I - r * nf);                                              // interface between cells f-1 and f of the row
-        j = (int)(r % g.n[1]); kz = (int)(r / g.n[1]);
+        unflatten3(I, nf, g.n[1], g.idx32, f, j, kz);                       // f: interface between cells f-1 and f of row (j, kz)
         p = f + (long long)(j + g.h[1]) * g.es[1] + (long long)(kz + g.h[2]) * g.es[2];    // extended index of cell f-1
         double A[5], B[5];
 #ifdef MF_STRICT
@@ -439,7 +436,11 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
             double acc = sF[v][t + 1] - F[v];
             if (g.act[1]) acc = acc + (fx.f[1][v][pc] - fx.f[1][v][pc - g.es[1]]);
             if (g.act[2]) acc = acc + (fx.f[2][v][pc] - fx.f[2][v][pc - g.es[2]]);
+#ifdef MF_STRICT
             double L = -acc / g.dx;                                        // Eq.1 :43
+#else
+            double L = -acc * g.inv_dx;
+#endif
             if (src.on && v < 2) L = L + S;
             const double ua = FORM == 3 ? 0.0 : Ua.q[v][o];
             const double ub = (FORM == 1 || FORM == 2) ? Ub.q[v][o] : 0.0;

@@ -241,7 +241,11 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
 #pragma unroll
                 for (int v = 0; v < 5; ++v) {
                     double acc = s_xy[v][t] + (F[v] - s_Fz[v][t]);
+#ifdef MF_STRICT
                     double L = -acc / g.dx;
+#else
+                    double L = -acc * g.inv_dx;
+#endif
                     if (src.on && v < 2) L = L + S;
                     double ua = sg.form == 3 ? 0.0 : Ua.q[v][o];
                     double ub = (sg.form == 1 || sg.form == 2) ? V.q[v][o] : 0.0;

@@ -17,6 +17,8 @@ struct Grid {
     long long ns[3];   // strides of the interior layout
     long long es[3];   // strides of the extended layout
     double dx;
+    double inv_dx;     // 1/dx: the product build multiplies, the strict build divides like the oracle
+    int idx32;         // every index space of this grid is below 2^31: kernels split indices with 32-bit divisions
 };
 
 // Per-step scalars that live in device memory so that a step never needs the host (A10).
