@@ -78,8 +78,8 @@ def alg_bytes(rk):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch group at 256^3 (config 3, staged path), one ncu --set full capture:
-# k_cell_stage 0.683 + 2.709 GB; k_flux_stage<1>, <2> 2.033 + 2.034 GB; k_xflux_combine 4.097 + 0.817 GB (profiles/r01_ncu_full_staged_256.md)
-NCU_TRAFFIC_GB_256 = {"cell_stage": 3.392, "flux_stage": 4.067, "combine": 4.914}
+# k_cell_stage 3.393 GB; k_flux_stage<1>, <2> 2.033 + 2.038 GB; k_xflux_combine 4.721 GB (profiles/r01_ncu_full_staged_256.md)
+NCU_TRAFFIC_GB_256 = {"cell_stage": 3.393, "flux_stage": 4.071, "combine": 4.721}
 
 FP64_LANES_PER_SM = 64       # B200 (sm_100): 4 SMSPs x 16 FP64 lanes; mf_probe_fp64 measures it
 
@@ -106,11 +106,16 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "--id=%d" % self.index, "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                          "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except OSError:
             self.proc = None
+
+    def wait_first(self, timeout_s):
+        t_end = time.perf_counter() + timeout_s
+        while self.proc is not None and not self.lines and time.perf_counter() < t_end:
+            time.sleep(0.01)
 
     def _read(self):
         for line in self.proc.stdout:
@@ -254,12 +259,13 @@ def run_ours(args):
         dev = [torch.from_numpy(np.ascontiguousarray(st[f])).to("cuda", non_blocking=False) for f in fields]
         stream.synchronize()
         g.set_state_device([t.data_ptr() for t in dev])
+        sampler = ClockSampler(local_rank)                        # started before the warm-up: nvidia-smi needs ~0.2 s to deliver its first line
+        sampler.start()
+        sampler.wait_first(3.0)
         g.step(args.warmup, st["cfl"])
         g.sync()
         rep.barrier()
         torch.cuda.synchronize()
-        sampler = ClockSampler(local_rank)
-        sampler.start()
         l0 = g.launch_count()
         g.profile(True)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
