@@ -54,7 +54,8 @@ enum { MF_PATH_AUTO = 0   /* fastest path that supports the configuration */,
        MF_PATH_HYBRID = 3 /* the staged cell stage + the tile kernel (3D grids) */ };
 
 /* Create a context for an nx*ny*nz grid of spacing dx (same on every axis).  An axis of extent 1 is inactive
- * (ny = nz = 1 is the 1D scheme); an active axis needs extent >= 4.  0 <= k_stages <= 8 is the number of Eq.8
+ * (ny = nz = 1 is the 1D scheme); an active axis needs extent >= 4; the grid with its boundary layer must have fewer
+ * than 2^32 cells (the 400 B/cell of HBM are the tighter limit).  0 <= k_stages <= 8 is the number of Eq.8
  * updates (FORCE is evaluated k_stages+1 times, reading A5).  Defaults: RK2, outflow, cs2 = 1/3, Hancock
  * predictor on, alpha = number of active axes (:151), no source.  Returns NULL on bad arguments, allocation
  * failure or missing GPU (mf_last_error(NULL) tells which). */

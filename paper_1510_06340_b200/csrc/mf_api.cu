@@ -297,6 +297,10 @@ mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k
     g.periodic = 0;
     g.ncell = (long long)nx * ny * nz;
     g.next = (long long)g.e[0] * g.e[1] * g.e[2];
+    if (g.next >= (1LL << 32)) {                                    // the kernels index cells with unsigned 32-bit offsets
+        fail(nullptr, MF_EINVAL, "grid has 2^32 or more cells");
+        delete c; return nullptr;
+    }
     g.ns[0] = 1; g.ns[1] = nx; g.ns[2] = (long long)nx * ny;
     g.es[0] = 1; g.es[1] = g.e[0]; g.es[2] = (long long)g.e[0] * g.e[1];
     g.dx = dx;

@@ -122,7 +122,11 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
     int cc[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) cc[a] = g.act[a] ? bc_index(c[a], g.n[a], g.periodic) : 0;
-    const long long o0 = cc[0] * g.ns[0] + cc[1] * g.ns[1] + cc[2] * g.ns[2];
+    // every offset fits 32 bits (mf_create refuses grids of 2^32 cells or more - 400 B/cell of HBM is the tighter limit); unsigned
+    // 32-bit offsets make each address one IMAD.WIDE.U32 instead of a 64-bit add pair
+    const unsigned int ns[3] = { (unsigned int)g.ns[0], (unsigned int)g.ns[1], (unsigned int)g.ns[2] };
+    const unsigned int o0 = cc[0] * ns[0] + cc[1] * ns[1] + cc[2] * ns[2];
+    const unsigned int pu = (unsigned int)p;
     double U0[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) U0[v] = V.q[v][o0];
@@ -132,8 +136,8 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         if (!g.act[d]) continue;
-        const long long om = o0 + (long long)(bc_index(c[d] - 1, g.n[d], g.periodic) - cc[d]) * g.ns[d];
-        const long long op = o0 + (long long)(bc_index(c[d] + 1, g.n[d], g.periodic) - cc[d]) * g.ns[d];
+        const unsigned int om = o0 + (unsigned int)(bc_index(c[d] - 1, g.n[d], g.periodic) - cc[d]) * ns[d];
+        const unsigned int op = o0 + (unsigned int)(bc_index(c[d] + 1, g.n[d], g.periodic) - cc[d]) * ns[d];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
             double a = U0[v] - V.q[v][om];
@@ -176,7 +180,7 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
     for (int d = 0; d < 3; ++d) {
         if (!g.act[d]) continue;
 #pragma unroll
-        for (int v = 0; v < 5; ++v) { fc.f[d][0][v][p] = UL[d][v]; fc.f[d][1][v][p] = UR[d][v]; }
+        for (int v = 0; v < 5; ++v) { fc.f[d][0][v][pu] = UL[d][v]; fc.f[d][1][v][pu] = UR[d][v]; }
     }
 #else
     // Product build, compact scratch (160 instead of 240 B/cell in 3D): the half slopes H_d = slope_d/2 per direction and
@@ -188,8 +192,8 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             if (!g.act[d]) continue;
-            const long long om = o0 + (long long)(bc_index(c[d] - 1, g.n[d], g.periodic) - cc[d]) * g.ns[d];
-            const long long op = o0 + (long long)(bc_index(c[d] + 1, g.n[d], g.periodic) - cc[d]) * g.ns[d];
+            const unsigned int om = o0 + (unsigned int)(bc_index(c[d] - 1, g.n[d], g.periodic) - cc[d]) * ns[d];
+            const unsigned int op = o0 + (unsigned int)(bc_index(c[d] + 1, g.n[d], g.periodic) - cc[d]) * ns[d];
 #pragma unroll
             for (int v = 0; v < 5; ++v) { Um[d][v] = __ldg(&V.q[v][om]); Up[d][v] = __ldg(&V.q[v][op]); }
         }
@@ -200,8 +204,8 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
             for (int v = 0; v < 5; ++v) {
                 double a = U0[v] - Um[d][v];
                 double b = Up[d][v] - U0[v];
-                H[d][v] = 0.5 * slope2<LIM>(a, b);                         // Eq.15-17, Eq.12
-                fc.f[d][0][v][p] = H[d][v];
+                H[d][v] = half_slope2<LIM>(a, b);                           // Eq.15-17, Eq.12
+                fc.f[d][0][v][pu] = H[d][v];
             }
         }
     }
@@ -238,7 +242,7 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
     }
     const int dW = g.act[0] ? 0 : (g.act[1] ? 1 : 2);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) fc.f[dW][1][v][p] = W[v];
+    for (int v = 0; v < 5; ++v) fc.f[dW][1][v][pu] = W[v];
 #endif
 }
 
