@@ -305,7 +305,7 @@ mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k
     g.es[0] = 1; g.es[1] = g.e[0]; g.es[2] = (long long)g.e[0] * g.e[1];
     g.dx = dx;
     g.inv_dx = 1.0 / dx;
-    g.idx32 = g.next < (1LL << 31);
+    for (int a = 0; a < 2; ++a) for (int m = 0; m < 3; ++m) g.dv[a][m] = make_fastdiv((unsigned int)(n[a] + m));
     set_eos(c->q, 1.0 / 3.0);
     clear_table(c->q);
     c->eos = eos; c->table = nullptr;

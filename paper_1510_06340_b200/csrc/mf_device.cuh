@@ -369,17 +369,18 @@ __device__ __forceinline__ double signal_speed(const Eos& q, double E, double Mx
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
-// idx -> (a, b, c) with idx = a + n0*(b + n1*c).  64-bit division costs ~100 instructions on the GPU; every index space of a grid below
-// 2^31 cells (Grid::idx32, set by mf_create) is split with two 32-bit divisions instead.
-__device__ __forceinline__ void unflatten3(long long idx, int n0, int n1, int idx32, int& a, int& b, int& c)
+// idx -> (a, b, c) with idx = a + d0*(b + d1*c), idx < 2^32 (mf_create refuses larger grids), by two multiply-shift divisions.
+template <class FD>
+__device__ __forceinline__ unsigned int fastdiv(unsigned int n, const FD& f)
 {
-    if (idx32) {
-        const unsigned int u = (unsigned int)idx, r = u / (unsigned int)n0, q2 = r / (unsigned int)n1;
-        a = (int)(u - r * (unsigned int)n0); b = (int)(r - q2 * (unsigned int)n1); c = (int)q2;
-    } else {
-        const long long r = idx / n0, q2 = r / n1;
-        a = (int)(idx - r * n0); b = (int)(r - q2 * n1); c = (int)q2;
-    }
+    const unsigned int t = __umulhi(f.mul, n);
+    return (t + ((n - t) >> f.sh1)) >> f.sh2;
+}
+template <class FD>
+__device__ __forceinline__ void unflatten3(unsigned int idx, const FD& d0, const FD& d1, int& a, int& b, int& c)
+{
+    const unsigned int r = fastdiv(idx, d0), q2 = fastdiv(r, d1);
+    a = (int)(idx - r * d0.d); b = (int)(r - q2 * d1.d); c = (int)q2;
 }
 
 __device__ __forceinline__ int bc_index(int i, int n, int periodic)

@@ -20,7 +20,7 @@ __global__ void __launch_bounds__(TPB_D) k_delta_stage(Grid g, Eos q, CState5 V,
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= g.next) return;
     int ie, je, ke;
-    unflatten3(p, g.e[0], g.e[1], g.idx32, ie, je, ke);
+    unflatten3((unsigned int)p, g.dv[0][2 * g.h[0]], g.dv[1][2 * g.h[1]], ie, je, ke);
     const int cx = ie - 1, cy = je - 1, cz = ke - 1;
     const int per = g.periodic;
     const long long ox0 = bc_index(cx, g.n[0], per), oxm = bc_index(cx - 1, g.n[0], per), oxp = bc_index(cx + 1, g.n[0], per);

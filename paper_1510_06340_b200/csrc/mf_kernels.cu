@@ -117,7 +117,7 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= g.next) return;
     int ie, je, ke;
-    unflatten3(p, g.e[0], g.e[1], g.idx32, ie, je, ke);
+    unflatten3((unsigned int)p, g.dv[0][2 * g.h[0]], g.dv[1][2 * g.h[1]], ie, je, ke);
     const int c[3] = { ie - g.h[0], je - g.h[1], ke - g.h[2] };             // interior coordinates, may be -1 or n
     int cc[3];
 #pragma unroll
@@ -270,17 +270,18 @@ __global__ void __launch_bounds__(TPB, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q,
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= total) return;
     int c[3];
-    unflatten3(t, m[0], m[1], g.idx32, c[0], c[1], c[2]);
+    unflatten3((unsigned int)t, g.dv[0][D == 0], g.dv[1][D == 1], c[0], c[1], c[2]);
     c[D] -= 1;
-    const long long p = (c[0] + g.h[0]) * g.es[0] + (c[1] + g.h[1]) * g.es[1] + (c[2] + g.h[2]) * g.es[2];
+    const unsigned int es[3] = { (unsigned int)g.es[0], (unsigned int)g.es[1], (unsigned int)g.es[2] };
+    const unsigned int p = (c[0] + g.h[0]) * es[0] + (c[1] + g.h[1]) * es[1] + (c[2] + g.h[2]) * es[2];   // < 2^32 (mf_create)
     double A[5], B[5], F[5];
 #pragma unroll
 #ifdef MF_STRICT
-    for (int v = 0; v < 5; ++v) { A[v] = fc.f[D][1][v][p]; B[v] = fc.f[D][0][v][p + g.es[D]]; }   // A2 :173
+    for (int v = 0; v < 5; ++v) { A[v] = fc.f[D][1][v][p]; B[v] = fc.f[D][0][v][p + es[D]]; }   // A2 :173
 #else
     {                                                                                             // compact scratch: W and H_D
         const int dW = g.act[0] ? 0 : (g.act[1] ? 1 : 2);
-        const long long pn = p + g.es[D];
+        const unsigned int pn = p + es[D];
 #pragma unroll
         for (int v = 0; v < 5; ++v) { A[v] = fc.f[dW][1][v][p] + fc.f[D][0][v][p]; B[v] = fc.f[dW][1][v][pn] - fc.f[D][0][v][pn]; }
     }
@@ -336,7 +337,7 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
     int bad = 0;
     if (o < g.ncell) {
         int i, j, k;
-        unflatten3(o, g.n[0], g.n[1], g.idx32, i, j, k);
+        unflatten3((unsigned int)o, g.dv[0][0], g.dv[1][0], i, j, k);
         const long long p = (i + g.h[0]) * g.es[0] + (j + g.h[1]) * g.es[1] + (k + g.h[2]) * g.es[2];
         const double dt = ds->dt;
         double S = 0.0;
@@ -398,11 +399,11 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
     const long long I = (long long)blockIdx.x * (TPB - 1) + t;
     const bool live = I < nrows * nf;
     int f = 0, j = 0, kz = 0;
-    long long p = 0;
+    unsigned int p = 0;                                                      // cell offsets fit 32 bits (mf_create)
     double F[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
     if (live) {
-        unflatten3(I, nf, g.n[1], g.idx32, f, j, kz);                       // f: interface between cells f-1 and f of row (j, kz)
-        p = f + (long long)(j + g.h[1]) * g.es[1] + (long long)(kz + g.h[2]) * g.es[2];    // extended index of cell f-1
+        unflatten3((unsigned int)I, g.dv[0][1], g.dv[1][0], f, j, kz);                       // f: interface between cells f-1 and f of row (j, kz)
+        p = f + (unsigned int)(j + g.h[1]) * (unsigned int)g.es[1] + (unsigned int)(kz + g.h[2]) * (unsigned int)g.es[2];    // extended index of cell f-1
         double A[5], B[5];
 #ifdef MF_STRICT
 #pragma unroll
@@ -412,7 +413,7 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
         for (int v = 0; v < 5; ++v) { A[v] = fc.f[0][1][v][p] + fc.f[0][0][v][p]; B[v] = fc.f[0][1][v][p + 1] - fc.f[0][0][v][p + 1]; }
 #endif
         if (t < TPB - 1 && f < g.n[0]) {                                    // pull the combine's operands towards L2 while MUSTA runs
-            const long long pc = p + 1, o = f + (long long)j * g.ns[1] + (long long)kz * g.ns[2];
+            const unsigned int pc = p + 1, o = f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
 #pragma unroll
             for (int v = 0; v < 5; ++v) {
                 if (g.act[1]) prefetch_l2(&fx.f[1][v][pc]);      // the neighbour lines (pc - es) are somebody else's pc: prefetching
@@ -429,8 +430,8 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
     double smax = 0.0;
     int bad = 0;
     if (live && t < TPB - 1 && f < g.n[0]) {                                // cell (f, j, kz): lower x face = this interface, upper = thread t+1's
-        const long long pc = p + 1;
-        const long long o = f + (long long)j * g.ns[1] + (long long)kz * g.ns[2];
+        const unsigned int pc = p + 1;
+        const unsigned int o = f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
         const double dt = ds->dt;
         double S = 0.0;
         if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
@@ -438,8 +439,8 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
             double acc = sF[v][t + 1] - F[v];
-            if (g.act[1]) acc = acc + (fx.f[1][v][pc] - fx.f[1][v][pc - g.es[1]]);
-            if (g.act[2]) acc = acc + (fx.f[2][v][pc] - fx.f[2][v][pc - g.es[2]]);
+            if (g.act[1]) acc = acc + (fx.f[1][v][pc] - fx.f[1][v][pc - (unsigned int)g.es[1]]);
+            if (g.act[2]) acc = acc + (fx.f[2][v][pc] - fx.f[2][v][pc - (unsigned int)g.es[2]]);
 #ifdef MF_STRICT
             double L = -acc / g.dx;                                        // Eq.1 :43
 #else

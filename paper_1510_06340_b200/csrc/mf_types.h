@@ -5,6 +5,24 @@
 
 namespace mf {
 
+// Division of an unsigned 32-bit index by a divisor fixed at mf_create (Granlund-Montgomery round-up multiplier): q = n / d for
+// every n < 2^32 in five integer instructions; the general '/' costs ~20 (32-bit) or ~100 (64-bit) on the GPU.
+struct FastDiv {
+    unsigned int d, mul;
+    int sh1, sh2;
+};
+inline FastDiv make_fastdiv(unsigned int d)
+{
+    FastDiv f;
+    int l = 0;
+    while ((1ull << l) < d) ++l;                                   // ceil(log2 d)
+    f.d = d;
+    f.mul = (unsigned int)(((1ull << 32) * ((1ull << l) - d)) / d + 1);
+    f.sh1 = l < 1 ? l : 1;
+    f.sh2 = l > 1 ? l - 1 : 0;
+    return f;
+}
+
 // Grid geometry, passed to kernels by value.
 struct Grid {
     int n[3];          // interior extents (x, y, z)
@@ -18,7 +36,7 @@ struct Grid {
     long long es[3];   // strides of the extended layout
     double dx;
     double inv_dx;     // 1/dx: the product build multiplies, the strict build divides like the oracle
-    int idx32;         // every index space of this grid is below 2^31: kernels split indices with 32-bit divisions
+    FastDiv dv[2][3];  // dv[a][m]: division by n[a] + m, a = x, y, m = 0, 1, 2: every row length an index space of this grid has
 };
 
 // Per-step scalars that live in device memory so that a step never needs the host (A10).
