@@ -103,6 +103,7 @@ void set_eos(Eos& q, double cs2)
 void clear_table(Eos& q)
 {
     q.kind = 0; q.ne = q.nn = 0; q.pad = 0; q.ln_e0 = q.dln_e = q.n0 = q.dn = 0.0; q.lnp = nullptr;
+    q.inv_dln_e = q.inv_dn = 0.0; q.lnpf = nullptr;
 }
 
 int resolve_path(mf_ctx* c)
@@ -626,11 +627,18 @@ int mf_set_eos_table(mf_ctx* c, int ne, int nn, double ln_e0, double dln_e, doub
     if (ne < 2 || nn < 1 || !(dln_e > 0.0) || (nn > 1 && !(dn > 0.0)) || !ln_p) return fail(c, MF_EINVAL, "bad table");
     MF_CUDA(c, cudaStreamSynchronize(c->stream));
     if (c->table) { cudaFree(c->table); c->table = nullptr; }
-    const size_t bytes = sizeof(double) * (size_t)ne * nn;
-    if (cudaMalloc(&c->table, bytes) != cudaSuccess) { cudaGetLastError(); c->table = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(EOS table) failed"); }
+    const size_t count = (size_t)ne * nn, bytes = sizeof(double) * count;
+    if (cudaMalloc(&c->table, bytes + sizeof(float) * count) != cudaSuccess) { cudaGetLastError(); c->table = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(EOS table) failed"); }
     MF_CUDA(c, cudaMemcpy(c->table, ln_p, bytes, cudaMemcpyHostToDevice));
+    {                                                  // float copy behind the doubles: the fp32 seed of the speed solve reads it
+        std::vector<float> lf(count);
+        for (size_t i = 0; i < count; ++i) lf[i] = (float)ln_p[i];
+        MF_CUDA(c, cudaMemcpy(c->table + count, lf.data(), sizeof(float) * count, cudaMemcpyHostToDevice));
+    }
     c->q.kind = 1; c->q.ne = ne; c->q.nn = nn; c->q.ln_e0 = ln_e0; c->q.dln_e = dln_e; c->q.n0 = n0; c->q.dn = nn > 1 ? dn : 1.0;
     c->q.lnp = c->table;
+    c->q.lnpf = reinterpret_cast<const float*>(c->table + count);
+    c->q.inv_dln_e = 1.0 / c->q.dln_e; c->q.inv_dn = 1.0 / c->q.dn;
     c->smax_valid = 0;
     return MF_OK;
 }

@@ -26,6 +26,9 @@ struct Eos {
     int kind, ne, nn, pad;
     double ln_e0, dln_e, n0, dn;
     const double* lnp;
+    // product build: reciprocal spacings and a float copy of ln p for the fp32 seed of the speed solve
+    double inv_dln_e, inv_dn;
+    const float* lnpf;
 };
 
 struct EosValue {
@@ -38,10 +41,13 @@ struct TableRef {
     const double* lnp;
     int ne, nn;
     double ln_e0, dln_e, n0, dn;
+    double inv_dln_e, inv_dn;
+    const float* lnpf;
 };
 __device__ __forceinline__ TableRef table_of(const Eos& q)
 {
     TableRef t; t.lnp = q.lnp; t.ne = q.ne; t.nn = q.nn; t.ln_e0 = q.ln_e0; t.dln_e = q.dln_e; t.n0 = q.n0; t.dn = q.dn;
+    t.inv_dln_e = q.inv_dln_e; t.inv_dn = q.inv_dn; t.lnpf = q.lnpf;
     return t;
 }
 
@@ -92,8 +98,163 @@ __device__ __forceinline__ EosValue eos_eval(const Eos& q, double e, double n)
 struct SpeedEP {
     double v, e, p;
 };
+#ifndef MF_STRICT
+// ---- product build: the same root in far fewer FP64 instructions.
+//  1. fp32 seed: the p = e/3 closed form, then two Newton steps on the float copy of the table (MUFU log/exp): |dv|/v ~ 1e-5.
+//  2. fp64 Newton from the seed.  The first evaluation pays log() and exp(); every later one moves e and ln p by a tiny
+//     relative amount, so ln e' = ln e + log1p(d) and p' = p exp(d') are three-term series (|d| < 1e-4, error < 3e-17).
+//  3. Quadratic convergence: once |dv| <= 3e-8 the step just taken is the last (error ~ dv^2), and p at the new speed is the
+//     first-order update with the derivative Newton already has.
+// Anything unusual (seed or step outside (0, |M|/E), no convergence in 4 steps, non-finite) falls back to the bracketed loop below.
+struct TableEvalState {
+    double e, inv_e, lne, lp, p, p_e, p_n;
+    int i, j;                                                  // table cell of the evaluation
+};
+
+__device__ __forceinline__ double rcp_pos(double x)            // 1/x, x normal and positive; 3 FP64 instructions, < 1 ulp
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e1 = fma(-x, y, 1.0);
+    return fma(y, fma(e1, e1, e1), y);
+}
+__device__ __forceinline__ double sqrt_newton(double x)        // sqrt(x), x normal and positive; 7 FP64 instructions
+{
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double g = x * r, h = 0.5 * r;
+    const double e1 = fma(-g, h, 0.5);
+    g = fma(g, e1, g); h = fma(h, e1, h);
+    return fma(h, fma(-g, g, x), g);
+}
+
+template <bool INCR>
+__device__ __forceinline__ void table_eval_step(const TableRef& q, double e, double n, TableEvalState& s)
+{
+    double lne;
+    if (INCR) {
+        const double d = (e - s.e) * s.inv_e;
+        lne = fabs(d) < 1e-4 ? fma(d, fma(d, fma(d, 1.0 / 3.0, -0.5), 1.0), s.lne) : log(e);
+    } else lne = log(e);
+    const double x = (lne - q.ln_e0) * q.inv_dln_e;
+    const int i = max(0, min(__double2int_rd(x), q.ne - 2));
+    const double fx = x - (double)i;
+    int j = 0;
+    double fy = 0.0;
+    bool n_inside = false;
+    if (q.nn > 1) {
+        const double y = (n - q.n0) * q.inv_dn;
+        j = max(0, min(__double2int_rd(y), q.nn - 2));
+        fy = y - (double)j;
+        n_inside = fy >= 0.0 && fy <= 1.0;
+        fy = fmin(fmax(fy, 0.0), 1.0);
+    }
+    const double* row0 = q.lnp + (unsigned int)(j * q.ne + i);
+    const double* row1 = q.nn > 1 ? row0 + q.ne : row0;
+    const double l00 = __ldg(row0), l10 = __ldg(row1);
+    const double d0 = __ldg(row0 + 1) - l00, d1 = __ldg(row1 + 1) - l10;
+    const double l0 = fma(fx, d0, l00), l1 = fma(fx, d1, l10);
+    const double lp = fma(fy, l1 - l0, l0);
+    double p;
+    if (INCR) {
+        const double d = lp - s.lp;
+        p = fabs(d) < 1e-4 ? s.p * fma(d, fma(d, fma(d, 1.0 / 6.0, 0.5), 1.0), 1.0) : exp(lp);
+    } else p = exp(lp);
+    const double inv_e = rcp_pos(e);
+    s.e = e; s.inv_e = inv_e; s.lne = lne; s.lp = lp; s.p = p; s.i = i; s.j = j;
+    s.p_e = p * (fma(fy, d1 - d0, d0) * q.inv_dln_e) * inv_e;
+    s.p_n = n_inside ? p * ((l1 - l0) * q.inv_dn) : 0.0;
+}
+
+// fp32 seed of the speed: p = e/3 closed form, then two Newton steps on the float table.  Any float in [0, hi] is a valid seed.
+__device__ __forceinline__ float seed_speed_f32(const TableRef& q, float E, float M, float R, float hi)
+{
+    const float c1 = 4.0f / 3.0f;
+    float v = __fdividef(2.0f * M, fmaf(c1, E, sqrtf(fmaxf(fmaf(c1 * c1 * E, E, -c1 * M * M), 0.0f))));
+    const float ln_e0 = (float)q.ln_e0, inv_dln_e = (float)q.inv_dln_e, n0 = (float)q.n0, inv_dn = (float)q.inv_dn;
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const float e = fmaf(-M, v, E);
+        const float g2 = fmaf(-v, v, 1.0f);
+        if (!(e > 0.0f) || !(g2 > 0.0f)) break;
+        const float rg = rsqrtf(g2), g = g2 * rg;
+        const float x = (__logf(e) - ln_e0) * inv_dln_e;
+        const int i = max(0, min(__float2int_rd(x), q.ne - 2));
+        const float fx = x - (float)i;
+        int j = 0;
+        float fy = 0.0f;
+        bool n_inside = false;
+        if (q.nn > 1) {
+            const float y = (R * g - n0) * inv_dn;
+            j = max(0, min(__float2int_rd(y), q.nn - 2));
+            fy = y - (float)j;
+            n_inside = fy >= 0.0f && fy <= 1.0f;
+            fy = fminf(fmaxf(fy, 0.0f), 1.0f);
+        }
+        const float* row0 = q.lnpf + (unsigned int)(j * q.ne + i);
+        const float* row1 = q.nn > 1 ? row0 + q.ne : row0;
+        const float l00 = __ldg(row0), l10 = __ldg(row1);
+        const float d0 = __ldg(row0 + 1) - l00, d1 = __ldg(row1 + 1) - l10;
+        const float l0 = fmaf(fx, d0, l00), l1 = fmaf(fx, d1, l10);
+        const float p = __expf(fmaf(fy, l1 - l0, l0));
+        const float p_e = __fdividef(p * fmaf(fy, d1 - d0, d0) * inv_dln_e, e);
+        const float p_n = n_inside ? p * (l1 - l0) * inv_dn : 0.0f;
+        const float f = fmaf(v, E + p, -M);
+        const float df = E + p - v * fmaf(M, p_e, R * v * rg * p_n);
+        const float vn = v - __fdividef(f, df);
+        if (!(vn >= 0.0f && vn <= hi)) break;
+        v = vn;
+    }
+    return v;
+}
+
+__device__ __forceinline__ bool solve_speed_fast(const TableRef& q, double E, double M, double R, double& v_out, double& e_out, double& p_out)
+{
+    const double hi = M * rcp_pos(E);
+    double v = (double)seed_speed_f32(q, (float)E, (float)M, (float)R, (float)hi);
+    if (!(v > 0.0 && v < hi)) return false;
+    TableEvalState s;
+#pragma unroll 1
+    for (int it = 0; it < 6; ++it) {
+        const double e = fma(-M, v, E);
+        const double g = sqrt_newton(fma(-v, v, 1.0));
+        if (it == 0) table_eval_step<false>(q, e, R * g, s); else table_eval_step<true>(q, e, R * g, s);
+        const double f = fma(v, E + s.p, -M);
+        const double dpdv = -fma(M, s.p_e, R * (v * rcp_pos(g)) * s.p_n);
+        const double df = fma(v, dpdv, E + s.p);
+        const double dv = -f * rcp_pos(df);
+        const double vn = v + dv;
+        if (!(df > 0.0) || !(vn > 0.0 && vn < hi)) return false;
+        if (fabs(dv) <= 3e-8) {
+            // the step is the last one if p is smooth between v and vn, i.e. both lie in one table cell (ln p has kinks at the cell
+            // edges, across which Newton converges only linearly), or if it is as small as the bracketed loop's own stopping step
+            const double en = fma(-M, vn, E);
+            const double d = (en - s.e) * s.inv_e;
+            bool last = fabs(dv) <= 1e-15;
+            if (!last && fabs(d) < 1e-4) {
+                const double lne = fma(d, fma(d, fma(d, 1.0 / 3.0, -0.5), 1.0), s.lne);
+                last = max(0, min(__double2int_rd((lne - q.ln_e0) * q.inv_dln_e), q.ne - 2)) == s.i;
+                if (last && q.nn > 1) {
+                    const double gn = sqrt_newton(fma(-vn, vn, 1.0));
+                    last = max(0, min(__double2int_rd((R * gn - q.n0) * q.inv_dn), q.nn - 2)) == s.j;
+                }
+            }
+            if (last) { v_out = vn; e_out = en; p_out = fma(dpdv, dv, s.p); return true; }
+        }
+        v = vn;
+    }
+    return false;
+}
+#endif
+
 static __device__ __noinline__ SpeedEP solve_speed(TableRef q, double E, double M, double R)
 {
+#ifndef MF_STRICT
+    {
+        SpeedEP r;
+        if (solve_speed_fast(q, E, M, R, r.v, r.e, r.p)) return r;
+    }
+#endif
     double lo = 0.0, hi = M / E, v = hi;
     for (int it = 0; it < 60; ++it) {
         const double e = E - M * v;
