@@ -103,9 +103,11 @@ struct SpeedEP {
 //  1. fp32 seed: the p = e/3 closed form, then two Newton steps on the float copy of the table (MUFU log/exp): |dv|/v ~ 1e-5.
 //  2. fp64 Newton from the seed.  The first evaluation pays log() and exp(); every later one moves e and ln p by a tiny
 //     relative amount, so ln e' = ln e + log1p(d) and p' = p exp(d') are three-term series (|d| < 1e-4, error < 3e-17).
-//  3. Quadratic convergence: once |dv| <= 3e-8 the step just taken is the last (error ~ dv^2), and p at the new speed is the
-//     first-order update with the derivative Newton already has.
-// Anything unusual (seed or step outside (0, |M|/E), no convergence in 4 steps, non-finite) falls back to the bracketed loop below.
+//  3. Quadratic convergence: once |dv| <= 3e-8 the step just taken is the last (error ~ dv^2) provided p is smooth between the two
+//     speeds, i.e. both lie in one table cell (ln p has kinks at the cell edges, across which Newton converges only linearly);
+//     p at the new speed is then the first-order update with the derivative Newton already has.
+// Anything unusual (seed or step outside (0, |M|/E), no convergence in 6 steps, non-finite) falls back to the bracketed loop below.
+// The solve stays a non-inlined call: inlined into the kernels it measured 15% slower (B200, 128^3), at 80 and at 128 registers.
 struct TableEvalState {
     double e, inv_e, lne, lp, p, p_e, p_n;
     int i, j;                                                  // table cell of the evaluation
