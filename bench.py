@@ -155,6 +155,20 @@ def make_workload(args):
     return st
 
 
+def batch_fields(args, st):
+    """The state arrays of the run: one event, or --batch B events stacked event-major for mf_create_batch (config 4: the seeded events
+    0..B-1 of the 32; any other config: B copies of its state)."""
+    fields = ("E", "Mx", "My", "Mz", "R")
+    if args.batch <= 1:
+        return [np.ascontiguousarray(st[f]) for f in fields]
+    if args.config == 4:
+        shape = tuple(int(x) for x in args.grid.split(",")) if args.grid else None
+        events = [st] + [workloads.lumpy_event(event=ev, shape=shape) for ev in range(1, args.batch)]
+    else:
+        events = [st] * args.batch
+    return [np.ascontiguousarray(np.stack([ev[f] for ev in events])) for f in fields]
+
+
 def describe(st, extra=None):
     nz, ny, nx = st["shape"]
     cfg = {"workload": "%s %dx%dx%d dx=%g %s k=%d RK%d %s cfl=%g" % (
@@ -243,20 +257,23 @@ def run_ours(args):
     rep = Replicas(backend="nccl", device=torch.device("cuda", local_rank))
     st = make_workload(args)
     nz, ny, nx = st["shape"]
-    cells = nx * ny * nz
+    nbatch = max(1, args.batch)
+    cells = nx * ny * nz * nbatch
     sch = st["scheme"]
     ndim = sum(1 for n in (nx, ny, nz) if n > 1)
+    arrays = batch_fields(args, st)
 
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         eos_table = workloads.crossover_eos_table() if args.eos == "table" else None     # 8(f) row 1; not the metric's workload
-        g = MustaForce(nx, ny, nz, dx=st["dx"], path=args.path, stream=stream.cuda_stream, eos_table=eos_table, **sch)
+        g = MustaForce(nx, ny, nz, dx=st["dx"], path=args.path, stream=stream.cuda_stream, eos_table=eos_table,
+                       batch=nbatch if nbatch > 1 else None, **sch)
         if "jet" in st:
             j = st["jet"]
             g.set_jet_source(j["dEdx"], j["sigma"], j["x0"], j["y0"], j["z0"])
         fields = ("E", "Mx", "My", "Mz", "R")
         # device-resident inputs for the kernel-throughput leg
-        dev = [torch.from_numpy(np.ascontiguousarray(st[f])).to("cuda", non_blocking=False) for f in fields]
+        dev = [torch.from_numpy(a).to("cuda", non_blocking=False) for a in arrays]
         stream.synchronize()
         g.set_state_device([t.data_ptr() for t in dev])
         sampler = ClockSampler(local_rank)                        # started before the warm-up: nvidia-smi needs ~0.2 s to deliver its first line
@@ -286,7 +303,7 @@ def run_ours(args):
         value = rep.sum(cells * args.steps) / (elapsed_ms * 1e-3)
 
         # ---- end to end through the C ABI with HOST buffers: H2D of the step's input and D2H of its result inside the timed region
-        pin_in = [torch.from_numpy(np.ascontiguousarray(st[f])).pin_memory() for f in fields]
+        pin_in = [torch.from_numpy(a).pin_memory() for a in arrays]
         pin_out = [torch.empty_like(t).pin_memory() for t in pin_in]
         np_in = [t.numpy() for t in pin_in]
         np_out = [t.numpy() for t in pin_out]
@@ -347,6 +364,7 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "config": describe(st, {"path": g.path(), "l2": "state registers (%.0f MB each) exceed the 126 MB L2" % (40e-6 * cells)
                                     if 40 * cells > 126e6 else "state fits in L2 (small grid)", "parallelism": "replicas x%d" % world,
+                                    "batch": "%d events per launch (mf_create_batch), each on its own dt" % nbatch if nbatch > 1 else "single event",
                                     "status": status, "eos": "p = e/3 (closed-form con2prim)" if args.eos == "cs2" else
                                     "tabulated crossover p(e,n), Newton con2prim (roofline fractions below use the closed-form slot count)"}),
             "clocks": clocks,
@@ -377,6 +395,7 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid"])
     ap.add_argument("--eos", default="cs2", choices=["cs2", "table"], help="table: synthetic crossover p(e,n) table with Newton con2prim")
     ap.add_argument("--predictor", default="on", choices=["on", "off"], help="off: without the Hancock half step (reading A4), reported beside the default")
+    ap.add_argument("--batch", type=int, default=1, help="events per context (mf_create_batch); config 4: the seeded events 0..B-1")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--ref-crop", type=int, default=64, help="edge of the centred crop the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -62,6 +62,15 @@ enum { MF_PATH_AUTO = 0   /* fastest path that supports the configuration */,
 mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k_stages);
 void    mf_destroy(mf_ctx*);
 
+/* A batch of nevents independent events on identical grids (event-by-event running is what the paper builds the code for, :25, :389;
+ * SURVEY.md 8(f) row 4): every kernel launch covers all events, each event keeps its own time and - under mf_step - its own
+ * dt = cfl*dx/S_max(event) on the device, so an event of the batch evolves exactly as it would alone in an mf_create context.
+ * Every state array of the calls below then holds nevents*nx*ny*nz doubles, event-major: idx = cell + nx*ny*nz*event.  Scheme options
+ * (limiter, RK, boundary, EOS, source, ...) are shared by the batch.  1 <= nevents <= 65535, nevents*(cells with boundary layer) < 2^32;
+ * runs on the staged path.  mf_create(...) is mf_create_batch(1, ...). */
+mf_ctx* mf_create_batch(int nevents, int nx, int ny, int nz, double dx, int eos, int limiter, int k_stages);
+int mf_batch_size(mf_ctx*);                 /* nevents (1 for mf_create) */
+
 /* Copy a conserved state in (5 HOST arrays) and reset t = 0, steps = 0, status = MF_OK.  Synchronous. */
 int mf_set_state(mf_ctx*, const double* E, const double* Mx, const double* My, const double* Mz, const double* R);
 /* Copy the conserved state out (5 HOST arrays).  Synchronises; returns MF_ESTATE if the sticky flag is up. */
@@ -78,11 +87,15 @@ int mf_get_state_prim(mf_ctx*, double* e, double* vx, double* vy, double* vz, do
 int mf_step(mf_ctx*, int n, double cfl);
 int mf_step_dt(mf_ctx*, int n, double dt);
 
-/* out[q] = dx^D * sum over cells of (E, Mx, My, Mz, R), D = number of active axes.  Synchronises. */
+/* out[q] = dx^D * sum over cells of (E, Mx, My, Mz, R), D = number of active axes; over all events of a batch, or over one.
+ * Synchronises. */
 int mf_conserved_totals(mf_ctx*, double out[5]);
-/* Simulation time, last dt used, steps taken since mf_set_state.  Any pointer may be NULL.  Synchronises. */
+int mf_conserved_totals_event(mf_ctx*, int event, double out[5]);
+/* Simulation time, last dt used, steps taken since mf_set_state (of event 0 / of the given event: under mf_step the events of a
+ * batch run on their own clocks).  Any pointer may be NULL.  Synchronises. */
 int mf_get_time(mf_ctx*, double* t, double* last_dt, long long* steps);
-/* S_max of the stored state (runs the CFL reduction).  Synchronises. */
+int mf_get_time_event(mf_ctx*, int event, double* t, double* last_dt, long long* steps);
+/* S_max of the stored state (runs the CFL reduction); the largest over the events of a batch.  Synchronises. */
 int mf_max_signal_speed(mf_ctx*, double* smax);
 
 int mf_set_rk(mf_ctx*, int order);          /* 2 (Eq.6, default) or 3 (Eq.7) */

@@ -25,6 +25,8 @@ _v5 = [_vp] * 5
 # name -> (restype, argtypes); the list is checked against include/mustaforce.h by tests/test_abi.py
 SIGNATURES = {
     "mf_create": (_vp, [C.c_int] * 3 + [C.c_double] + [C.c_int] * 3),
+    "mf_create_batch": (_vp, [C.c_int] * 4 + [C.c_double] + [C.c_int] * 3),
+    "mf_batch_size": (C.c_int, [_vp]),
     "mf_destroy": (None, [_vp]),
     "mf_set_state": (C.c_int, [_vp] + _d5),
     "mf_get_state": (C.c_int, [_vp] + _d5),
@@ -35,7 +37,9 @@ SIGNATURES = {
     "mf_step": (C.c_int, [_vp, C.c_int, C.c_double]),
     "mf_step_dt": (C.c_int, [_vp, C.c_int, C.c_double]),
     "mf_conserved_totals": (C.c_int, [_vp, _dp]),
+    "mf_conserved_totals_event": (C.c_int, [_vp, C.c_int, _dp]),
     "mf_get_time": (C.c_int, [_vp, _dp, _dp, C.POINTER(C.c_longlong)]),
+    "mf_get_time_event": (C.c_int, [_vp, C.c_int, _dp, _dp, C.POINTER(C.c_longlong)]),
     "mf_max_signal_speed": (C.c_int, [_vp, _dp]),
     "mf_set_rk": (C.c_int, [_vp, C.c_int]),
     "mf_set_boundary": (C.c_int, [_vp, C.c_int]),
@@ -105,15 +109,21 @@ def version(strict=False):
 
 
 class MustaForce:
-    """One mf_ctx.  Host arrays are numpy float64, shape (nz, ny, nx) or flat, x fastest."""
+    """One mf_ctx.  Host arrays are numpy float64, shape (nz, ny, nx) or flat, x fastest; with batch=B (mf_create_batch: B independent
+    events stepped by the same launches, each on its own clock) every array has shape (B, nz, ny, nx)."""
 
     def __init__(self, nx, ny=1, nz=1, dx=1.0, limiter="minmod", k_stages=2, rk=2, bc="outflow", predictor=True,
-                 alpha=None, cs2=None, path="auto", stream=None, strict=False, eos_table=None):
+                 alpha=None, cs2=None, path="auto", stream=None, strict=False, eos_table=None, batch=None):
         self.lib = load(strict)
-        self.shape = (nz, ny, nx)
-        self.n = nx * ny * nz
+        self.batch = batch
+        self.shape = (nz, ny, nx) if batch is None else (int(batch), nz, ny, nx)
+        self.n = nx * ny * nz * (1 if batch is None else int(batch))
         lim = LIM[limiter] if isinstance(limiter, str) else int(limiter)
-        self.h = self.lib.mf_create(nx, ny, nz, float(dx), MF_EOS_CS2 if eos_table is None else MF_EOS_TABLE, lim, int(k_stages))
+        eos = MF_EOS_CS2 if eos_table is None else MF_EOS_TABLE
+        if batch is None:
+            self.h = self.lib.mf_create(nx, ny, nz, float(dx), eos, lim, int(k_stages))
+        else:
+            self.h = self.lib.mf_create_batch(int(batch), nx, ny, nz, float(dx), eos, lim, int(k_stages))
         if not self.h:
             raise MustaForceError(MF_EINVAL, self.lib.mf_last_error(None).decode())
         self._chk(self.lib.mf_set_rk(self.h, int(rk)))
@@ -178,15 +188,21 @@ class MustaForce:
     def sync(self):
         return self._chk(self.lib.mf_sync(self.h), allow=(MF_ESTATE,))
 
-    def totals(self):
+    def totals(self, event=None):
         out = np.empty(5)
-        self._chk(self.lib.mf_conserved_totals(self.h, _p(out)), allow=(MF_ESTATE,))
+        if event is None:
+            self._chk(self.lib.mf_conserved_totals(self.h, _p(out)), allow=(MF_ESTATE,))
+        else:
+            self._chk(self.lib.mf_conserved_totals_event(self.h, int(event), _p(out)), allow=(MF_ESTATE,))
         return out
 
-    def time(self):
+    def time(self, event=0):
         t, dt, s = C.c_double(), C.c_double(), C.c_longlong()
-        self._chk(self.lib.mf_get_time(self.h, C.byref(t), C.byref(dt), C.byref(s)), allow=(MF_ESTATE,))
+        self._chk(self.lib.mf_get_time_event(self.h, int(event), C.byref(t), C.byref(dt), C.byref(s)), allow=(MF_ESTATE,))
         return t.value, dt.value, s.value
+
+    def batch_size(self):
+        return self.lib.mf_batch_size(self.h)
 
     def max_signal_speed(self):
         s = C.c_double()

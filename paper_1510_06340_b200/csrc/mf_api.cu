@@ -28,7 +28,9 @@ struct mf_ctx {
     int path_req, path;
     int dev, num_sms;
     cudaStream_t own_stream, stream;
-    double* U[3];            // three state registers, 5*ncell doubles each (U^n, U_(1), U_(2)), component-major
+    int nev;                 // events in the batch (1 unless mf_create_batch)
+    long long nst, nxt;      // nev*ncell, nev*next: the length of one component array in the interior / extended layout
+    double* U[3];            // three state registers, 5*nst doubles each (U^n, U_(1), U_(2)), component-major, [component][event][cell]
     int cur;                 // which register holds U^n
     double* faces;           // staged path: 2*5*nact*next doubles
     double* fluxes;          // staged path: 5*nact*next doubles
@@ -36,7 +38,7 @@ struct mf_ctx {
     int eos;                 // MF_EOS_*
     double* table;           // tabulated EOS: ln p, device copy
     int smax_valid;          // the device-side S_max accumulator already holds the reduction of the current U^n (fused into the last combine)
-    StepState* ds;
+    StepState* ds;           // one per event
     StepState* h_ds;         // pinned mirror
     double* partials;        // totals: 5*nblocks doubles
     double* h_partials;
@@ -72,7 +74,7 @@ Faces faces_of(mf_ctx* c)
     long long slot = 0;
     for (int d = 0; d < 3; ++d) {
         if (!c->g.act[d]) continue;
-        for (int s = 0; s < 2; ++s) for (int v = 0; v < 5; ++v) f.f[d][s][v] = c->faces + (slot++) * c->g.next;
+        for (int s = 0; s < 2; ++s) for (int v = 0; v < 5; ++v) f.f[d][s][v] = c->faces + (slot++) * c->nxt;
     }
     return f;
 }
@@ -83,7 +85,7 @@ Fluxes fluxes_of(mf_ctx* c)
     long long slot = 0;
     for (int d = 0; d < 3; ++d) {
         if (!c->g.act[d]) continue;
-        for (int v = 0; v < 5; ++v) f.f[d][v] = c->fluxes + (slot++) * c->g.next;
+        for (int v = 0; v < 5; ++v) f.f[d][v] = c->fluxes + (slot++) * c->nxt;
     }
     return f;
 }
@@ -109,7 +111,7 @@ void clear_table(Eos& q)
 int resolve_path(mf_ctx* c)
 {
     if (c->path_req == MF_PATH_FUSED || c->path_req == MF_PATH_HYBRID) {
-        if (!fused_supported(c->g) || c->eos != MF_EOS_CS2) return MF_EINVAL;      // the tile kernel is built for p = cs2*e and three active axes
+        if (!fused_supported(c->g) || c->eos != MF_EOS_CS2 || c->nev > 1) return MF_EINVAL;      // the tile kernel is built for p = cs2*e and three active axes
         c->path = c->path_req;
     }
     else if (c->path_req == MF_PATH_STAGED) c->path = MF_PATH_STAGED;
@@ -143,7 +145,7 @@ void prof_end(mf_ctx* c, int slot)
 int ensure_staged_buffers(mf_ctx* c)
 {
     if (c->faces) return MF_OK;
-    size_t nf = (size_t)10 * c->nact * c->g.next, nx = (size_t)5 * c->nact * c->g.next;
+    size_t nf = (size_t)10 * c->nact * c->nxt, nx = (size_t)5 * c->nact * c->nxt;
     if (cudaMalloc(&c->faces, nf * sizeof(double)) != cudaSuccess) { cudaGetLastError(); c->faces = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(face states) failed"); }
     if (cudaMalloc(&c->fluxes, nx * sizeof(double)) != cudaSuccess) { cudaGetLastError(); cudaFree(c->faces); c->faces = nullptr; c->fluxes = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(fluxes) failed"); }
     return MF_OK;
@@ -152,7 +154,7 @@ int ensure_staged_buffers(mf_ctx* c)
 // One evaluation of  out = form(Ua, V, L(V) + S)  on the selected path.
 int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, double* out)
 {
-    const long long n = c->g.ncell;
+    const long long n = c->nst;
     if (c->path == MF_PATH_FUSED || c->path == MF_PATH_HYBRID) {
         if (c->path == MF_PATH_HYBRID) {                           // the staged path's cell stage + the tile kernel
             int rc = ensure_staged_buffers(c);
@@ -231,7 +233,7 @@ int run_step(mf_ctx* c)
         if ((rc = run_stage(c, Rb, s3, Un, Ra)) != MF_OK) return rc;
         c->cur = (c->cur + 1) % 3;
     }
-    c->launches += launch_end_step(c->ds, c->stream);
+    c->launches += launch_end_step(c->ds, c->nev, c->stream);
     c->smax_valid = c->path == MF_PATH_STAGED;
     return MF_OK;
 }
@@ -246,9 +248,11 @@ int check_launch(mf_ctx* c)
 // synchronise and fetch the device-side step state into the pinned mirror
 int fetch_step_state(mf_ctx* c)
 {
-    MF_CUDA(c, cudaMemcpyAsync(c->h_ds, c->ds, sizeof(StepState), cudaMemcpyDeviceToHost, c->stream));
+    MF_CUDA(c, cudaMemcpyAsync(c->h_ds, c->ds, sizeof(StepState) * c->nev, cudaMemcpyDeviceToHost, c->stream));
     MF_CUDA(c, cudaStreamSynchronize(c->stream));
-    if (c->h_ds->status) return fail(c, MF_ESTATE, "a CFL reduction met a non-finite or superluminal (|M| > E) cell");
+    int status = 0;
+    for (int ev = 0; ev < c->nev; ++ev) status |= c->h_ds[ev].status;
+    if (status) return fail(c, MF_ESTATE, "a CFL reduction met a non-finite or superluminal (|M| > E) cell");
     return MF_OK;
 }
 
@@ -260,7 +264,13 @@ const char* mf_version(void) { return MF_VERSION_STR; }
 
 mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k_stages)
 {
+    return mf_create_batch(1, nx, ny, nz, dx, eos, limiter, k_stages);
+}
+
+mf_ctx* mf_create_batch(int nevents, int nx, int ny, int nz, double dx, int eos, int limiter, int k_stages)
+{
     const int n[3] = { nx, ny, nz };
+    if (nevents < 1 || nevents > 65535) { fail(nullptr, MF_EINVAL, "the number of events must be in 1..65535"); return nullptr; }
     for (int a = 0; a < 3; ++a)
         if (n[a] < 1 || (n[a] > 1 && n[a] < 4)) { fail(nullptr, MF_EINVAL, "each extent must be 1 (inactive) or >= 4"); return nullptr; }
     if (!(dx > 0.0)) { fail(nullptr, MF_EINVAL, "dx must be > 0"); return nullptr; }
@@ -298,7 +308,9 @@ mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k
     g.periodic = 0;
     g.ncell = (long long)nx * ny * nz;
     g.next = (long long)g.e[0] * g.e[1] * g.e[2];
-    if (g.next >= (1LL << 32)) {                                    // the kernels index cells with unsigned 32-bit offsets
+    g.nev = c->nev = nevents;
+    c->nst = g.ncell * nevents; c->nxt = g.next * nevents;
+    if (c->nxt >= (1LL << 32)) {                                    // the kernels index cells with unsigned 32-bit offsets
         fail(nullptr, MF_EINVAL, "grid has 2^32 or more cells");
         delete c; return nullptr;
     }
@@ -320,14 +332,14 @@ mf_ctx* mf_create(int nx, int ny, int nz, double dx, int eos, int limiter, int k
 
     bool ok = cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) == cudaSuccess;
     c->stream = c->own_stream;
-    for (int r = 0; ok && r < 3; ++r) ok = cudaMalloc(&c->U[r], sizeof(double) * 5 * g.ncell) == cudaSuccess;
-    ok = ok && cudaMalloc(&c->ds, sizeof(StepState)) == cudaSuccess;
-    ok = ok && cudaMallocHost(&c->h_ds, sizeof(StepState)) == cudaSuccess;
+    for (int r = 0; ok && r < 3; ++r) ok = cudaMalloc(&c->U[r], sizeof(double) * 5 * c->nst) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->ds, sizeof(StepState) * nevents) == cudaSuccess;
+    ok = ok && cudaMallocHost(&c->h_ds, sizeof(StepState) * nevents) == cudaSuccess;
     ok = ok && cudaMalloc(&c->partials, sizeof(double) * 5 * c->nblocks_tot) == cudaSuccess;
     ok = ok && cudaMallocHost(&c->h_partials, sizeof(double) * 5 * c->nblocks_tot) == cudaSuccess;
     if (ok) {
-        for (int r = 0; r < 3; ++r) cudaMemsetAsync(c->U[r], 0, sizeof(double) * 5 * g.ncell, c->stream);
-        c->launches += launch_reset(c->ds, c->stream);
+        for (int r = 0; r < 3; ++r) cudaMemsetAsync(c->U[r], 0, sizeof(double) * 5 * c->nst, c->stream);
+        c->launches += launch_reset(c->ds, c->nev, c->stream);
         ok = cudaStreamSynchronize(c->stream) == cudaSuccess;
     }
     if (!ok) {
@@ -418,7 +430,7 @@ namespace {
 int reset_after_set(mf_ctx* c)
 {
     c->smax_valid = 0;
-    c->launches += launch_reset(c->ds, c->stream);
+    c->launches += launch_reset(c->ds, c->nev, c->stream);
     return check_launch(c);
 }
 
@@ -426,14 +438,14 @@ int copy_in(mf_ctx* c, const double* const src[5], cudaMemcpyKind kind)
 {
     c->cur = 0;
     for (int v = 0; v < 5; ++v)
-        MF_CUDA(c, cudaMemcpyAsync(c->U[0] + v * c->g.ncell, src[v], sizeof(double) * c->g.ncell, kind, c->stream));
+        MF_CUDA(c, cudaMemcpyAsync(c->U[0] + v * c->nst, src[v], sizeof(double) * c->nst, kind, c->stream));
     return MF_OK;
 }
 
 int copy_out(mf_ctx* c, const double* base, double* const dst[5], cudaMemcpyKind kind)
 {
     for (int v = 0; v < 5; ++v)
-        MF_CUDA(c, cudaMemcpyAsync(dst[v], base + v * c->g.ncell, sizeof(double) * c->g.ncell, kind, c->stream));
+        MF_CUDA(c, cudaMemcpyAsync(dst[v], base + v * c->nst, sizeof(double) * c->nst, kind, c->stream));
     return MF_OK;
 }
 
@@ -490,7 +502,7 @@ int mf_set_state_prim(mf_ctx* c, const double* e, const double* vx, const double
     const double* src[5] = { e, vx, vy, vz, n };
     int rc = copy_in(c, src, cudaMemcpyHostToDevice);
     if (rc != MF_OK) return rc;
-    c->launches += launch_prim2con(c->g, c->q, state(c->U[0], c->g.ncell), c->stream);      // Eq.4 on the device
+    c->launches += launch_prim2con(c->g, c->q, state(c->U[0], c->nst), c->stream);      // Eq.4 on the device
     if ((rc = reset_after_set(c)) != MF_OK) return rc;
     MF_CUDA(c, cudaStreamSynchronize(c->stream));
     return MF_OK;
@@ -501,7 +513,7 @@ int mf_get_state_prim(mf_ctx* c, double* e, double* vx, double* vy, double* vz, 
     if (!c) return MF_EINVAL;
     if (!e || !vx || !vy || !vz || !n) return fail(c, MF_EINVAL, "null pointer");
     double* scratch = c->U[(c->cur + 1) % 3];
-    c->launches += launch_con2prim(c->g, c->q, cstate(c->U[c->cur], c->g.ncell), state(scratch, c->g.ncell), c->stream);
+    c->launches += launch_con2prim(c->g, c->q, cstate(c->U[c->cur], c->nst), state(scratch, c->nst), c->stream);
     int rc = check_launch(c);
     if (rc != MF_OK) return rc;
     double* dst[5] = { e, vx, vy, vz, n };
@@ -516,10 +528,10 @@ int mf_step(mf_ctx* c, int n, double cfl)
     for (int s = 0; s < n; ++s) {
         if (!c->smax_valid) {                                      // otherwise the previous step's last combine already reduced U^n
             int ps = prof_begin(c, 0);
-            c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->g.ncell), c->ds, c->num_sms, c->stream);   // a2, from U^n
+            c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->nst), c->ds, c->num_sms, c->stream);   // a2, from U^n
             prof_end(c, ps);
         }
-        c->launches += launch_begin_step(c->ds, 0, cfl, c->g.dx, c->alpha, c->stream);
+        c->launches += launch_begin_step(c->ds, c->nev, 0, cfl, c->g.dx, c->alpha, c->stream);
         int rc = run_step(c);
         if (rc != MF_OK) return rc;
     }
@@ -531,7 +543,7 @@ int mf_step_dt(mf_ctx* c, int n, double dt)
     if (!c) return MF_EINVAL;
     if (n < 0 || !(dt > 0.0)) return fail(c, MF_EINVAL, "bad n or dt");
     for (int s = 0; s < n; ++s) {
-        c->launches += launch_begin_step(c->ds, 1, dt, c->g.dx, c->alpha, c->stream);
+        c->launches += launch_begin_step(c->ds, c->nev, 1, dt, c->g.dx, c->alpha, c->stream);
         int rc = run_step(c);
         if (rc != MF_OK) return rc;
     }
@@ -544,7 +556,7 @@ int mf_eval_L(mf_ctx* c, double dt, double* L_E, double* L_Mx, double* L_My, dou
     if (!(dt > 0.0) || !L_E || !L_Mx || !L_My || !L_Mz || !L_R) return fail(c, MF_EINVAL, "bad dt or null pointer");
     double* Un = c->U[c->cur];
     double* scratch = c->U[(c->cur + 1) % 3];
-    c->launches += launch_begin_step(c->ds, 1, dt, c->g.dx, c->alpha, c->stream);
+    c->launches += launch_begin_step(c->ds, c->nev, 1, dt, c->g.dx, c->alpha, c->stream);
     Stage sg = { 3, 0.0, 0.0, 0.0, 0.0 };
     c->smax_valid = 0;
     Source keep = c->src;
@@ -559,10 +571,14 @@ int mf_eval_L(mf_ctx* c, double dt, double* L_E, double* L_Mx, double* L_My, dou
     return MF_OK;
 }
 
-int mf_conserved_totals(mf_ctx* c, double out[5])
+// event < 0: all events of the batch
+static int totals_of(mf_ctx* c, int event, double out[5])
 {
-    if (!c || !out) return MF_EINVAL;
-    c->launches += launch_totals(c->g, cstate(c->U[c->cur], c->g.ncell), c->partials, c->nblocks_tot, c->stream);
+    Grid g = c->g;
+    CState5 U = cstate(c->U[c->cur], c->nst);
+    if (event < 0) g.ncell = c->nst;
+    else for (int v = 0; v < 5; ++v) U.q[v] += (long long)event * g.ncell;
+    c->launches += launch_totals(g, U, c->partials, c->nblocks_tot, c->stream);
     int rc = check_launch(c);
     if (rc != MF_OK) return rc;
     MF_CUDA(c, cudaMemcpyAsync(c->h_partials, c->partials, sizeof(double) * 5 * c->nblocks_tot, cudaMemcpyDeviceToHost, c->stream));
@@ -577,28 +593,47 @@ int mf_conserved_totals(mf_ctx* c, double out[5])
     return rc;
 }
 
-int mf_get_time(mf_ctx* c, double* t, double* last_dt, long long* steps)
+int mf_conserved_totals(mf_ctx* c, double out[5])
+{
+    if (!c || !out) return MF_EINVAL;
+    return totals_of(c, -1, out);
+}
+
+int mf_conserved_totals_event(mf_ctx* c, int event, double out[5])
+{
+    if (!c || !out) return MF_EINVAL;
+    if (event < 0 || event >= c->nev) return fail(c, MF_EINVAL, "no such event");
+    return totals_of(c, event, out);
+}
+
+int mf_batch_size(mf_ctx* c) { return c ? c->nev : MF_EINVAL; }
+
+int mf_get_time_event(mf_ctx* c, int event, double* t, double* last_dt, long long* steps)
 {
     if (!c) return MF_EINVAL;
+    if (event < 0 || event >= c->nev) return fail(c, MF_EINVAL, "no such event");
     int rc = fetch_step_state(c);
-    if (t) *t = c->h_ds->t;
-    if (last_dt) *last_dt = c->h_ds->dt;
-    if (steps) *steps = c->h_ds->steps;
+    if (t) *t = c->h_ds[event].t;
+    if (last_dt) *last_dt = c->h_ds[event].dt;
+    if (steps) *steps = c->h_ds[event].steps;
     return rc;
 }
+
+int mf_get_time(mf_ctx* c, double* t, double* last_dt, long long* steps) { return mf_get_time_event(c, 0, t, last_dt, steps); }
 
 int mf_max_signal_speed(mf_ctx* c, double* smax)
 {
     if (!c || !smax) return MF_EINVAL;
-    c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->g.ncell), c->ds, c->num_sms, c->stream);
+    c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->nst), c->ds, c->num_sms, c->stream);
     int rc = check_launch(c);
     if (rc != MF_OK) return rc;
     rc = fetch_step_state(c);
-    unsigned long long bits = c->h_ds->smax_bits;
+    unsigned long long bits = 0;                                   // non-negative doubles: bit order == value order
+    for (int ev = 0; ev < c->nev; ++ev) if (c->h_ds[ev].smax_bits > bits) bits = c->h_ds[ev].smax_bits;
     memcpy(smax, &bits, sizeof(double));
-    // leave the accumulator empty for the next reduction
+    // leave the accumulators empty for the next reduction
     c->smax_valid = 0;
-    cudaMemsetAsync(&c->ds->smax_bits, 0, sizeof(unsigned long long), c->stream);
+    for (int ev = 0; ev < c->nev; ++ev) cudaMemsetAsync(&c->ds[ev].smax_bits, 0, sizeof(unsigned long long), c->stream);
     return rc;
 }
 

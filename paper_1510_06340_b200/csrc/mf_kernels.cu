@@ -51,26 +51,34 @@ __global__ void __launch_bounds__(TPB) k_cfl(Grid g, Eos q, CState5 U, StepState
 {
     double smax = 0.0;
     int bad = 0;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < g.ncell; o += stride) {
+    const unsigned int eo = blockIdx.y * (unsigned int)g.ncell;       // this block's event
+    const unsigned int stride = gridDim.x * blockDim.x;
+    for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < (unsigned int)g.ncell; i += stride) {
+        const unsigned int o = eo + i;
         double s = signal_speed<EK>(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], U.q[4][o], bad);
         smax = fmax(smax, s);
     }
-    block_reduce_smax(smax, bad, ds);
+    block_reduce_smax(smax, bad, ds + blockIdx.y);
 }
 
 int launch_cfl(const Grid& g, const Eos& q, CState5 U, StepState* ds, int num_sms, cudaStream_t st)
 {
     unsigned int nb = blocks_for(g.ncell, TPB);
-    unsigned int cap = (unsigned int)num_sms * 8u;
+    unsigned int cap = (unsigned int)num_sms * 8u / (unsigned int)g.nev;
+    if (cap < 1u) cap = 1u;
     if (nb > cap) nb = cap;
-    if (q.kind) k_cfl<1><<<nb, TPB, 0, st>>>(g, q, U, ds); else k_cfl<0><<<nb, TPB, 0, st>>>(g, q, U, ds);
+    const dim3 grid(nb, g.nev);
+    if (q.kind) k_cfl<1><<<grid, TPB, 0, st>>>(g, q, U, ds); else k_cfl<0><<<grid, TPB, 0, st>>>(g, q, U, ds);
     return 1;
 }
 
 // =========================================================================== per-step scalars
-__global__ void k_begin_step(StepState* ds, int mode, double value, double dx, double alpha)
+// one thread per event of the batch
+__global__ void k_begin_step(StepState* ds, int nev, int mode, double value, double dx, double alpha)
 {
+    const int ev = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ev >= nev) return;
+    ds += ev;
     double dt;
     if (mode == 0) {
         double smax = __longlong_as_double((long long)ds->smax_bits);
@@ -87,25 +95,31 @@ __global__ void k_begin_step(StepState* ds, int mode, double value, double dx, d
     ds->smax_bits = 0ull;
 }
 
-__global__ void k_end_step(StepState* ds)
+__global__ void k_end_step(StepState* ds, int nev)
 {
+    const int ev = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ev >= nev) return;
+    ds += ev;
     ds->t = ds->t + ds->dt;
     ds->steps += 1;
 }
 
-__global__ void k_reset(StepState* ds)
+__global__ void k_reset(StepState* ds, int nev)
 {
+    const int ev = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ev >= nev) return;
+    ds += ev;
     ds->t = 0.0; ds->dt = 0.0; ds->lam = 0.0; ds->hl = 0.0; ds->c_lw = 0.0; ds->c_lf = 0.0;
     ds->smax_bits = 0ull; ds->status = 0; ds->pad = 0; ds->steps = 0;
 }
 
-int launch_begin_step(StepState* ds, int mode, double value, double dx, double alpha, cudaStream_t st)
+int launch_begin_step(StepState* ds, int nev, int mode, double value, double dx, double alpha, cudaStream_t st)
 {
-    k_begin_step<<<1, 1, 0, st>>>(ds, mode, value, dx, alpha);
+    k_begin_step<<<(nev + 63) / 64, nev < 64 ? nev : 64, 0, st>>>(ds, nev, mode, value, dx, alpha);
     return 1;
 }
-int launch_end_step(StepState* ds, cudaStream_t st) { k_end_step<<<1, 1, 0, st>>>(ds); return 1; }
-int launch_reset(StepState* ds, cudaStream_t st) { k_reset<<<1, 1, 0, st>>>(ds); return 1; }
+int launch_end_step(StepState* ds, int nev, cudaStream_t st) { k_end_step<<<(nev + 63) / 64, nev < 64 ? nev : 64, 0, st>>>(ds, nev); return 1; }
+int launch_reset(StepState* ds, int nev, cudaStream_t st) { k_reset<<<(nev + 63) / 64, nev < 64 ? nev : 64, 0, st>>>(ds, nev); return 1; }
 
 // =========================================================================== a3 + a4: cell stage
 // One thread per cell of the extended region (interior + 1 layer on every active axis).
@@ -125,8 +139,9 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
     // every offset fits 32 bits (mf_create refuses grids of 2^32 cells or more - 400 B/cell of HBM is the tighter limit); unsigned
     // 32-bit offsets make each address one IMAD.WIDE.U32 instead of a 64-bit add pair
     const unsigned int ns[3] = { (unsigned int)g.ns[0], (unsigned int)g.ns[1], (unsigned int)g.ns[2] };
-    const unsigned int o0 = cc[0] * ns[0] + cc[1] * ns[1] + cc[2] * ns[2];
-    const unsigned int pu = (unsigned int)p;
+    const unsigned int o0 = blockIdx.y * (unsigned int)g.ncell + cc[0] * ns[0] + cc[1] * ns[1] + cc[2] * ns[2];
+    const unsigned int pu = blockIdx.y * (unsigned int)g.next + (unsigned int)p;
+    ds += blockIdx.y;
     double U0[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) U0[v] = V.q[v][o0];
@@ -248,7 +263,7 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
 
 int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, CState5 V, Faces fc, const StepState* ds, cudaStream_t st)
 {
-    const unsigned int nb = blocks_for(g.next, TPB);
+    const dim3 nb(blocks_for(g.next, TPB), g.nev);
     switch (limiter) {
 #define MF_CASE(L) case L: if (q.kind) k_cell_stage<L, 1><<<nb, TPB, 0, st>>>(g, q, predictor, V, fc, ds); \
                            else k_cell_stage<L, 0><<<nb, TPB, 0, st>>>(g, q, predictor, V, fc, ds); break;
@@ -273,7 +288,8 @@ __global__ void __launch_bounds__(TPB, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q,
     unflatten3((unsigned int)t, g.dv[0][D == 0], g.dv[1][D == 1], c[0], c[1], c[2]);
     c[D] -= 1;
     const unsigned int es[3] = { (unsigned int)g.es[0], (unsigned int)g.es[1], (unsigned int)g.es[2] };
-    const unsigned int p = (c[0] + g.h[0]) * es[0] + (c[1] + g.h[1]) * es[1] + (c[2] + g.h[2]) * es[2];   // < 2^32 (mf_create)
+    const unsigned int p = blockIdx.y * (unsigned int)g.next + (c[0] + g.h[0]) * es[0] + (c[1] + g.h[1]) * es[1] + (c[2] + g.h[2]) * es[2];   // < 2^32 (mf_create)
+    ds += blockIdx.y;
     double A[5], B[5], F[5];
 #pragma unroll
 #ifdef MF_STRICT
@@ -298,7 +314,7 @@ int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, F
         if (!g.act[d] || !(dmask & (1 << d))) continue;
         long long total = 1;
         for (int a = 0; a < 3; ++a) total *= (a == d) ? g.n[a] + 1 : g.n[a];
-        unsigned int nb = blocks_for(total, TPB);
+        const dim3 nb(blocks_for(total, TPB), g.nev);
         if (d == 0) { if (q.kind) k_flux_stage<0, 1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<0, 0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); }
         if (d == 1) { if (q.kind) k_flux_stage<1, 1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<1, 0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); }
         if (d == 2) { if (q.kind) k_flux_stage<2, 1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<2, 0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); }
@@ -332,13 +348,16 @@ __device__ __forceinline__ double rk_form(const Stage& sg, double ua, double ub,
 template <int EK>
 __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds)
 {
-    const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long ol = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     double smax = 0.0;
     int bad = 0;
-    if (o < g.ncell) {
+    ds += blockIdx.y;
+    if (ol < g.ncell) {
         int i, j, k;
-        unflatten3((unsigned int)o, g.dv[0][0], g.dv[1][0], i, j, k);
-        const long long p = (i + g.h[0]) * g.es[0] + (j + g.h[1]) * g.es[1] + (k + g.h[2]) * g.es[2];
+        unflatten3((unsigned int)ol, g.dv[0][0], g.dv[1][0], i, j, k);
+        const unsigned int o = blockIdx.y * (unsigned int)g.ncell + (unsigned int)ol;
+        const unsigned int p = blockIdx.y * (unsigned int)g.next + (i + g.h[0]) * (unsigned int)g.es[0] + (j + g.h[1]) * (unsigned int)g.es[1]
+                               + (k + g.h[2]) * (unsigned int)g.es[2];
         const double dt = ds->dt;
         double S = 0.0;
         if (src.on) S = jet_source(g, src, i, j, k, ds->t + sg.ts * dt);
@@ -350,7 +369,7 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 if (!g.act[d]) continue;
-                double diff = fx.f[d][v][p] - fx.f[d][v][p - g.es[d]];
+                double diff = fx.f[d][v][p] - fx.f[d][v][p - (unsigned int)g.es[d]];
                 acc = first ? diff : acc + diff;
                 first = false;
             }
@@ -372,8 +391,9 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
 
 int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds, cudaStream_t st)
 {
-    if (q.kind) k_combine<1><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
-    else k_combine<0><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+    const dim3 nb(blocks_for(g.ncell, TPB), g.nev);
+    if (q.kind) k_combine<1><<<nb, TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+    else k_combine<0><<<nb, TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
     return 1;
 }
 
@@ -401,9 +421,11 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
     int f = 0, j = 0, kz = 0;
     unsigned int p = 0;                                                      // cell offsets fit 32 bits (mf_create)
     double F[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
+    const unsigned int eo = blockIdx.y * (unsigned int)g.ncell, ep = blockIdx.y * (unsigned int)g.next;   // this block's event
+    ds += blockIdx.y;
     if (live) {
         unflatten3((unsigned int)I, g.dv[0][1], g.dv[1][0], f, j, kz);                       // f: interface between cells f-1 and f of row (j, kz)
-        p = f + (unsigned int)(j + g.h[1]) * (unsigned int)g.es[1] + (unsigned int)(kz + g.h[2]) * (unsigned int)g.es[2];    // extended index of cell f-1
+        p = ep + f + (unsigned int)(j + g.h[1]) * (unsigned int)g.es[1] + (unsigned int)(kz + g.h[2]) * (unsigned int)g.es[2];   // extended index of cell f-1
         double A[5], B[5];
 #ifdef MF_STRICT
 #pragma unroll
@@ -413,7 +435,7 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
         for (int v = 0; v < 5; ++v) { A[v] = fc.f[0][1][v][p] + fc.f[0][0][v][p]; B[v] = fc.f[0][1][v][p + 1] - fc.f[0][0][v][p + 1]; }
 #endif
         if (t < TPB - 1 && f < g.n[0]) {                                    // pull the combine's operands towards L2 while MUSTA runs
-            const unsigned int pc = p + 1, o = f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
+            const unsigned int pc = p + 1, o = eo + f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
 #pragma unroll
             for (int v = 0; v < 5; ++v) {
                 if (g.act[1]) prefetch_l2(&fx.f[1][v][pc]);      // the neighbour lines (pc - es) are somebody else's pc: prefetching
@@ -431,7 +453,7 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
     int bad = 0;
     if (live && t < TPB - 1 && f < g.n[0]) {                                // cell (f, j, kz): lower x face = this interface, upper = thread t+1's
         const unsigned int pc = p + 1;
-        const unsigned int o = f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
+        const unsigned int o = eo + f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
         const double dt = ds->dt;
         double S = 0.0;
         if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
@@ -461,7 +483,7 @@ int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx
                          StepState* ds, cudaStream_t st)
 {
     const long long total = (long long)(g.n[0] + 1) * g.n[1] * g.n[2];
-    const unsigned int nb = blocks_for(total, TPB - 1);
+    const dim3 nb(blocks_for(total, TPB - 1), g.nev);
 #define MF_XFC(EK_, FORM_, CFL_) k_xflux_combine<EK_, FORM_, CFL_><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds)
 #define MF_XFC_FORMS(EK_) \
     if (sg.form == 0) { if (sg.cfl) MF_XFC(EK_, 0, true); else MF_XFC(EK_, 0, false); } \
@@ -478,8 +500,9 @@ int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx
 template <int EK>
 __global__ void __launch_bounds__(TPB) k_prim2con(Grid g, Eos q, State5 U)
 {
-    const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= g.ncell) return;
+    const long long ol = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (ol >= g.ncell) return;
+    const unsigned int o = blockIdx.y * (unsigned int)g.ncell + (unsigned int)ol;
     double e = U.q[0][o], vx = U.q[1][o], vy = U.q[2][o], vz = U.q[3][o], n = U.q[4][o];
     double p = eos_eval<EK>(q, e, n).p;                                // Eq.4 :63-67
     double g2 = 1.0 / (1.0 - (vx * vx + vy * vy + vz * vz));
@@ -490,8 +513,9 @@ __global__ void __launch_bounds__(TPB) k_prim2con(Grid g, Eos q, State5 U)
 template <int EK>
 __global__ void __launch_bounds__(TPB) k_con2prim(Grid g, Eos q, CState5 U, State5 P)
 {
-    const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= g.ncell) return;
+    const long long ol = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (ol >= g.ncell) return;
+    const unsigned int o = blockIdx.y * (unsigned int)g.ncell + (unsigned int)ol;
     double vx, vy, vz, e, p;
     velocity_pressure<EK>(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], U.q[4][o], vx, vy, vz, e, p);
     P.q[0][o] = e; P.q[1][o] = vx; P.q[2][o] = vy; P.q[3][o] = vz;
@@ -500,12 +524,14 @@ __global__ void __launch_bounds__(TPB) k_con2prim(Grid g, Eos q, CState5 U, Stat
 
 int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st)
 {
-    if (q.kind) k_prim2con<1><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U); else k_prim2con<0><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U);
+    const dim3 nb(blocks_for(g.ncell, TPB), g.nev);
+    if (q.kind) k_prim2con<1><<<nb, TPB, 0, st>>>(g, q, U); else k_prim2con<0><<<nb, TPB, 0, st>>>(g, q, U);
     return 1;
 }
 int launch_con2prim(const Grid& g, const Eos& q, CState5 U, State5 P, cudaStream_t st)
 {
-    if (q.kind) k_con2prim<1><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U, P); else k_con2prim<0><<<blocks_for(g.ncell, TPB), TPB, 0, st>>>(g, q, U, P);
+    const dim3 nb(blocks_for(g.ncell, TPB), g.nev);
+    if (q.kind) k_con2prim<1><<<nb, TPB, 0, st>>>(g, q, U, P); else k_con2prim<0><<<nb, TPB, 0, st>>>(g, q, U, P);
     return 1;
 }
 

@@ -8,9 +8,9 @@ namespace mf {
 // a2: CFL reduction of `U` into ds->smax_bits / ds->status (accumulator must have been reset by begin_step of the previous step or by reset_smax)
 int launch_cfl(const Grid& g, const Eos& q, CState5 U, StepState* ds, int num_sms, cudaStream_t st);
 // per-step scalars on the device: mode 0: dt = value*dx/smax (cfl), mode 1: dt = value (fixed); resets the smax accumulator
-int launch_begin_step(StepState* ds, int mode, double value, double dx, double alpha, cudaStream_t st);
-int launch_end_step(StepState* ds, cudaStream_t st);
-int launch_reset(StepState* ds, cudaStream_t st);
+int launch_begin_step(StepState* ds, int nev, int mode, double value, double dx, double alpha, cudaStream_t st);   // ds: one StepState per event
+int launch_end_step(StepState* ds, int nev, cudaStream_t st);
+int launch_reset(StepState* ds, int nev, cudaStream_t st);
 
 // ---- staged path (MF_PATH_STAGED): a3+a4, a5, a7(+a8) as three kernels, face states and fluxes through HBM
 int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, CState5 V, Faces fc, const StepState* ds, cudaStream_t st);

@@ -36,6 +36,8 @@ struct Grid {
     long long es[3];   // strides of the extended layout
     double dx;
     double inv_dx;     // 1/dx: the product build multiplies, the strict build divides like the oracle
+    int nev;           // events in the batch (mf_create_batch; 1 otherwise): blockIdx.y of every staged kernel is the event, whose cells
+                       // sit at offset event*ncell (interior layout) / event*next (extended layout) inside each component array
     FastDiv dv[2][3];  // dv[a][m]: division by n[a] + m, a = x, y, m = 0, 1, 2: every row length an index space of this grid has
 };
 
