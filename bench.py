@@ -67,6 +67,16 @@ def class_work(path, limiter, k, ndim, x_active, predictor=True):
         else:
             out["combine"] = (comb, 40 * ndim + 80 + 40)
         return out
+    if path == "sweep":
+        # the sweep kernels limit their own slopes (one direction's share of the reconstruction each) from U; with the predictor on a
+        # separate kernel writes delta (the reconstruction is then counted once more there: it is needed for Eq.13)
+        rdir = recon // ndim
+        dl = 40 if predictor else 0
+        out = {"flux_stage": ((ndim - 1) * (musta + rdir), (ndim - 1) * (40 + dl + 40)),          # U (+ delta) in, F_d out
+               "combine": (musta + rdir + comb, 40 + dl + 40 * (ndim - 1) + 40 + 40)}            # U (+ delta), F_y, F_z, U^n in; new state out
+        if predictor:
+            out["cell_stage"] = (recon + pred, 80)                                                 # U in, delta out
+        return out
     if path == "hybrid":
         return {"cell_stage": (recon + pred, 40 + 40 * (1 + ndim)), "fused_stage": (ndim * musta + comb, 40 + 40 * ndim + 80 + 40)}
     return {"cell_stage": (recon + pred, 80), "fused_stage": (recon + ndim * musta + comb, 80 + 80 + 40)}   # fused: delta kernel + tile kernel
@@ -392,7 +402,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (default 3 = the 256^3 metric workload)")
     ap.add_argument("--grid", default=None, help="nz,ny,nx override (parity/debug sizes)")
-    ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid"])
+    ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid", "sweep"])
     ap.add_argument("--eos", default="cs2", choices=["cs2", "table"], help="table: synthetic crossover p(e,n) table with Newton con2prim")
     ap.add_argument("--predictor", default="on", choices=["on", "off"], help="off: without the Hancock half step (reading A4), reported beside the default")
     ap.add_argument("--batch", type=int, default=1, help="events per context (mf_create_batch); config 4: the seeded events 0..B-1")

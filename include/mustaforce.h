@@ -51,7 +51,11 @@ enum { MF_OK = 0, MF_EINVAL = -1, MF_ENOMEM = -2, MF_ECUDA = -3, MF_ESTATE = -4 
 enum { MF_PATH_AUTO = 0   /* fastest path that supports the configuration */,
        MF_PATH_STAGED = 1 /* three kernels per RK stage, face states and fluxes through HBM */,
        MF_PATH_FUSED = 2  /* predictor kernel + one tile kernel per RK stage: face states, fluxes and differences on chip (3D grids) */,
-       MF_PATH_HYBRID = 3 /* the staged cell stage + the tile kernel (3D grids) */ };
+       MF_PATH_HYBRID = 3 /* the staged cell stage + the tile kernel (3D grids) */,
+       MF_PATH_SWEEP = 4  /* per-direction sweep kernels that limit the slopes themselves from a +-2-cell halo of the state (:33 "each dimension
+                             separately"): no face states in HBM.  Needs an active x axis and MF_EOS_CS2; with the Hancock predictor on also a
+                             3D grid and a single event (a predictor kernel then writes the increment of Eq.13 once per cell).  MF_PATH_AUTO
+                             takes it whenever the predictor is off. */ };
 
 /* Create a context for an nx*ny*nz grid of spacing dx (same on every axis).  An axis of extent 1 is inactive
  * (ny = nz = 1 is the 1D scheme); an active axis needs extent >= 4; the grid with its boundary layer must have fewer

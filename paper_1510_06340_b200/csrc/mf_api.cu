@@ -114,8 +114,16 @@ int resolve_path(mf_ctx* c)
         if (!fused_supported(c->g) || c->eos != MF_EOS_CS2 || c->nev > 1) return MF_EINVAL;      // the tile kernel is built for p = cs2*e and three active axes
         c->path = c->path_req;
     }
+    else if (c->path_req == MF_PATH_SWEEP) {
+        if (!sweep_supported(c->g, c->q.kind || c->eos != MF_EOS_CS2, c->predictor)) return MF_EINVAL;
+        c->path = MF_PATH_SWEEP;
+    }
     else if (c->path_req == MF_PATH_STAGED) c->path = MF_PATH_STAGED;
-    else c->path = MF_PATH_STAGED;      // measured faster than the fused path on B200 so far (profiles/)
+    else {
+        // AUTO.  Predictor on: the staged path measured faster than the fused path on B200 (profiles/).  Predictor off: the sweep kernels
+        // need no cell stage and no face-state scratch.
+        c->path = (!c->predictor && sweep_supported(c->g, c->q.kind || c->eos != MF_EOS_CS2, 0)) ? MF_PATH_SWEEP : MF_PATH_STAGED;
+    }
     return MF_OK;
 }
 
@@ -141,13 +149,28 @@ void prof_end(mf_ctx* c, int slot)
     c->prof_used = (size_t)slot + 1;
 }
 
-// staged path needs its scratch; allocate on first use so that the fused path keeps the footprint at 3 states
+// scratch is allocated on first use, so that a path only pays for what it needs (fused: delta; sweep: fluxes (+ delta); staged: faces + fluxes)
+int ensure_flux_buffer(mf_ctx* c)
+{
+    if (c->fluxes) return MF_OK;
+    size_t nx = (size_t)5 * c->nact * c->nxt;
+    if (cudaMalloc(&c->fluxes, nx * sizeof(double)) != cudaSuccess) { cudaGetLastError(); c->fluxes = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(fluxes) failed"); }
+    return MF_OK;
+}
+
+int ensure_delta_buffer(mf_ctx* c)
+{
+    if (c->delta) return MF_OK;
+    if (cudaMalloc(&c->delta, sizeof(double) * 5 * c->g.next) != cudaSuccess) { cudaGetLastError(); c->delta = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(delta) failed"); }
+    return MF_OK;
+}
+
 int ensure_staged_buffers(mf_ctx* c)
 {
-    if (c->faces) return MF_OK;
-    size_t nf = (size_t)10 * c->nact * c->nxt, nx = (size_t)5 * c->nact * c->nxt;
+    int rc = ensure_flux_buffer(c);
+    if (rc != MF_OK || c->faces) return rc;
+    size_t nf = (size_t)10 * c->nact * c->nxt;
     if (cudaMalloc(&c->faces, nf * sizeof(double)) != cudaSuccess) { cudaGetLastError(); c->faces = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(face states) failed"); }
-    if (cudaMalloc(&c->fluxes, nx * sizeof(double)) != cudaSuccess) { cudaGetLastError(); cudaFree(c->faces); c->faces = nullptr; c->fluxes = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(fluxes) failed"); }
     return MF_OK;
 }
 
@@ -168,9 +191,8 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
             prof_end(c, ps);
             return MF_OK;
         }
-        if (!c->delta) {
-            if (cudaMalloc(&c->delta, sizeof(double) * 5 * c->g.next) != cudaSuccess) { cudaGetLastError(); c->delta = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(delta) failed"); }
-        }
+        int rc = ensure_delta_buffer(c);
+        if (rc != MF_OK) return rc;
         int ps;
         if (c->predictor) {
             ps = prof_begin(c, 1);
@@ -180,6 +202,28 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
         ps = prof_begin(c, 4);
         c->launches += launch_fused_stage(c->g, c->q, c->limiter, c->predictor, c->k, cstate(V, n), cstate(c->delta, c->g.next), sg, cstate(Ua, n),
                                           state(out, n), c->src, c->ds, c->num_sms, 0, c->stream);
+        prof_end(c, ps);
+    } else if (c->path == MF_PATH_SWEEP) {
+        if (!sweep_supported(c->g, c->q.kind, c->predictor)) return fail(c, MF_EINVAL, "the sweep path does not support this configuration");
+        int rc = ensure_flux_buffer(c);
+        if (rc == MF_OK && c->predictor) rc = ensure_delta_buffer(c);
+        if (rc != MF_OK) return rc;
+        Fluxes fx = fluxes_of(c);
+        const bool pred = c->predictor != 0;
+        CState5 Dl = cstate(pred ? c->delta : V, pred ? c->g.next : n);
+        int ps;
+        if (pred) {
+            ps = prof_begin(c, 1);
+            c->launches += launch_delta_stage(c->g, c->q, c->limiter, cstate(V, n), state(c->delta, c->g.next), c->ds, c->stream);
+            prof_end(c, ps);
+        }
+        if (c->g.act[1] || c->g.act[2]) {
+            ps = prof_begin(c, 2);
+            c->launches += launch_sweep_flux(c->g, c->q, c->limiter, c->k, pred, cstate(V, n), Dl, fx, c->ds, c->stream);
+            prof_end(c, ps);
+        }
+        ps = prof_begin(c, 3);
+        c->launches += launch_sweep_xcombine(c->g, c->q, c->limiter, c->k, pred, cstate(V, n), Dl, fx, sg, cstate(Ua, n), state(out, n), c->src, c->ds, c->stream);
         prof_end(c, ps);
     } else {
         int rc = ensure_staged_buffers(c);
@@ -219,7 +263,7 @@ int run_step(mf_ctx* c)
     if (c->rk == 2) {
         Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
         Stage s2 = { 1, 0.5, 0.5, 1.0, 1.0 };
-        s2.cfl = c->path == MF_PATH_STAGED;
+        s2.cfl = c->path == MF_PATH_STAGED || c->path == MF_PATH_SWEEP;
         if ((rc = run_stage(c, Un, s1, Un, Ra)) != MF_OK) return rc;
         if ((rc = run_stage(c, Ra, s2, Un, Rb)) != MF_OK) return rc;
         c->cur = (c->cur + 2) % 3;
@@ -227,14 +271,14 @@ int run_step(mf_ctx* c)
         Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
         Stage s2 = { 2, 0.75, 0.25, 0.25, 1.0 };
         Stage s3 = { 2, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, 0.5 };
-        s3.cfl = c->path == MF_PATH_STAGED;
+        s3.cfl = c->path == MF_PATH_STAGED || c->path == MF_PATH_SWEEP;
         if ((rc = run_stage(c, Un, s1, Un, Ra)) != MF_OK) return rc;
         if ((rc = run_stage(c, Ra, s2, Un, Rb)) != MF_OK) return rc;
         if ((rc = run_stage(c, Rb, s3, Un, Ra)) != MF_OK) return rc;
         c->cur = (c->cur + 1) % 3;
     }
     c->launches += launch_end_step(c->ds, c->nev, c->stream);
-    c->smax_valid = c->path == MF_PATH_STAGED;
+    c->smax_valid = c->path == MF_PATH_STAGED || c->path == MF_PATH_SWEEP;
     return MF_OK;
 }
 
@@ -677,7 +721,14 @@ int mf_set_eos_table(mf_ctx* c, int ne, int nn, double ln_e0, double dln_e, doub
     c->smax_valid = 0;
     return MF_OK;
 }
-int mf_set_predictor(mf_ctx* c, int on) { if (!c) return MF_EINVAL; c->predictor = on ? 1 : 0; return MF_OK; }
+int mf_set_predictor(mf_ctx* c, int on)
+{
+    if (!c) return MF_EINVAL;
+    const int keep = c->predictor;
+    c->predictor = on ? 1 : 0;
+    if (resolve_path(c) != MF_OK) { c->predictor = keep; resolve_path(c); return fail(c, MF_EINVAL, "the selected path does not support this predictor setting: select another path first"); }
+    return MF_OK;
+}
 int mf_set_alpha(mf_ctx* c, double alpha)
 {
     if (!c) return MF_EINVAL;
@@ -700,10 +751,10 @@ int mf_set_jet_source(mf_ctx* c, double dEdx, double sigma, double x0, double y0
 int mf_set_path(mf_ctx* c, int path)
 {
     if (!c) return MF_EINVAL;
-    if (path < MF_PATH_AUTO || path > MF_PATH_HYBRID) return fail(c, MF_EINVAL, "unknown path");
+    if (path < MF_PATH_AUTO || path > MF_PATH_SWEEP) return fail(c, MF_EINVAL, "unknown path");
     int keep = c->path_req;
     c->path_req = path;
-    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "the fused path does not support this configuration (it needs three active axes and MF_EOS_CS2)"); }
+    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "this path does not support this configuration (fused/hybrid: three active axes, MF_EOS_CS2, one event; sweep: active x axis, MF_EOS_CS2, and with the predictor on a 3D grid and one event)"); }
     return MF_OK;
 }
 int mf_get_path(mf_ctx* c, int* path) { if (!c || !path) return MF_EINVAL; *path = c->path; return MF_OK; }

@@ -2,50 +2,32 @@
 // CFL reduction (a2), per-step scalars, cell stage (a3+a4), interface flux stage (a5+a6), combine (a7+a8),
 // prim<->con conversions, totals.  Boundary handling (a1) is index mapping in the loads: no stored ghosts.
 #include "mf_kernels.h"
+#include "mf_blocks.cuh"
 
 namespace mf {
 
-constexpr int TPB = 256;
+// threads per block / resident blocks per SM of the three hot kernels of the staged path (24 warps per SM at 80 registers)
+#ifndef MF_CELL_TPB
+#define MF_CELL_TPB 128
+#endif
+#ifndef MF_FLUX_TPB
+#define MF_FLUX_TPB 256
+#endif
+#ifndef MF_XC_TPB
+#define MF_XC_TPB 128
+#endif
 #ifndef MF_CELL_MINB
-#define MF_CELL_MINB 3
+#define MF_CELL_MINB (768 / MF_CELL_TPB)
 #endif
 #ifndef MF_FLUX_MINB
-#define MF_FLUX_MINB 3
+#define MF_FLUX_MINB (768 / MF_FLUX_TPB)
 #endif
+constexpr int CT = MF_CELL_TPB, FT = MF_FLUX_TPB, XT = MF_XC_TPB;
 
 static inline unsigned int blocks_for(long long n, int tpb) { return (unsigned int)((n + tpb - 1) / tpb); }
 
 
 // =========================================================================== a2: CFL reduction
-// warp shuffle max, then one value per warp through shared memory, then ONE atomic per block; every thread of the block must call it
-__device__ __forceinline__ void block_reduce_smax(double smax, int bad, StepState* ds)
-{
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, off));
-        bad |= __shfl_xor_sync(0xffffffffu, bad, off);
-    }
-    __shared__ double s_max[TPB / 32];
-    __shared__ int s_bad[TPB / 32];
-    const int tid = threadIdx.y * blockDim.x + threadIdx.x;          // TPB threads per block, whatever its shape
-    const int lane = tid & 31, warp = tid >> 5;
-    if (lane == 0) { s_max[warp] = smax; s_bad[warp] = bad; }
-    __syncthreads();
-    if (warp == 0) {
-        smax = lane < TPB / 32 ? s_max[lane] : 0.0;
-        bad = lane < TPB / 32 ? s_bad[lane] : 0;
-#pragma unroll
-        for (int off = 4; off > 0; off >>= 1) {
-            smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, off));
-            bad |= __shfl_xor_sync(0xffffffffu, bad, off);
-        }
-        if (lane == 0) {
-            atomicMax(&ds->smax_bits, (unsigned long long)__double_as_longlong(smax));   // smax >= 0: bit order == value order
-            if (bad) atomicOr(&ds->status, 1);
-        }
-    }
-}
-
 template <int EK>
 __global__ void __launch_bounds__(TPB) k_cfl(Grid g, Eos q, CState5 U, StepState* ds)
 {
@@ -124,7 +106,7 @@ int launch_reset(StepState* ds, int nev, cudaStream_t st) { k_reset<<<(nev + 63)
 // =========================================================================== a3 + a4: cell stage
 // One thread per cell of the extended region (interior + 1 layer on every active axis).
 template <int LIM, int EK>
-__global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, int predictor, CState5 V, Faces fc, const StepState* ds)
+__global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, int predictor, CState5 V, Faces fc, const StepState* ds)
 {
     // linear index over the extended region, x fastest: 256 consecutive cells per block (measured on B200: 32 x 8 tiles, which
     // reuse the y neighbours through L1, are 10-15% slower because the DRAM bursts get shorter)
@@ -263,10 +245,10 @@ __global__ void __launch_bounds__(TPB, MF_CELL_MINB) k_cell_stage(Grid g, Eos q,
 
 int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, CState5 V, Faces fc, const StepState* ds, cudaStream_t st)
 {
-    const dim3 nb(blocks_for(g.next, TPB), g.nev);
+    const dim3 nb(blocks_for(g.next, CT), g.nev);
     switch (limiter) {
-#define MF_CASE(L) case L: if (q.kind) k_cell_stage<L, 1><<<nb, TPB, 0, st>>>(g, q, predictor, V, fc, ds); \
-                           else k_cell_stage<L, 0><<<nb, TPB, 0, st>>>(g, q, predictor, V, fc, ds); break;
+#define MF_CASE(L) case L: if (q.kind) k_cell_stage<L, 1><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, ds); \
+                           else k_cell_stage<L, 0><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, ds); break;
         MF_CASE(LIM_NONE) MF_CASE(LIM_MINMOD) MF_CASE(LIM_SUPERBEE) MF_CASE(LIM_VANALBADA) MF_CASE(LIM_VANLEER) MF_CASE(LIM_MC) MF_CASE(LIM_FIRST)
 #undef MF_CASE
     default: return 0;
@@ -277,7 +259,7 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
 // =========================================================================== a5 + a6: interface fluxes
 // One thread per interface between cell c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
 template <int D, int EK>
-__global__ void __launch_bounds__(TPB, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, int k, Faces fc, Fluxes fx, const StepState* ds)
+__global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, int k, Faces fc, Fluxes fx, const StepState* ds)
 {
     int m[3] = { g.n[0], g.n[1], g.n[2] };
     m[D] += 1;
@@ -314,29 +296,16 @@ int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, F
         if (!g.act[d] || !(dmask & (1 << d))) continue;
         long long total = 1;
         for (int a = 0; a < 3; ++a) total *= (a == d) ? g.n[a] + 1 : g.n[a];
-        const dim3 nb(blocks_for(total, TPB), g.nev);
-        if (d == 0) { if (q.kind) k_flux_stage<0, 1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<0, 0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); }
-        if (d == 1) { if (q.kind) k_flux_stage<1, 1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<1, 0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); }
-        if (d == 2) { if (q.kind) k_flux_stage<2, 1><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<2, 0><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, ds); }
+        const dim3 nb(blocks_for(total, FT), g.nev);
+        if (d == 0) { if (q.kind) k_flux_stage<0, 1><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<0, 0><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); }
+        if (d == 1) { if (q.kind) k_flux_stage<1, 1><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<1, 0><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); }
+        if (d == 2) { if (q.kind) k_flux_stage<2, 1><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<2, 0><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); }
         ++launches;
     }
     return launches;
 }
 
 // =========================================================================== a7 + a8: divergence, source, RK combine
-__device__ __forceinline__ double jet_source(const Grid& g, const Source& s, int i, int j, int k, double t)
-{
-    double x = (i + 0.5 - g.n[0] / 2.0) * g.dx - (s.x0 + t);
-    double y = (j + 0.5 - g.n[1] / 2.0) * g.dx - s.y0;
-    double z = (k + 0.5 - g.n[2] / 2.0) * g.dx - s.z0;
-    double r2 = x * x + y * y + z * z;
-    double arg = -r2 * s.inv_two_s2;
-#ifndef MF_STRICT
-    if (arg < -745.0) return 0.0;            // exp underflows to 0 in fp64 anyway
-#endif
-    return s.dEdx * s.norm * exp(arg);
-}
-
 __device__ __forceinline__ double rk_form(const Stage& sg, double ua, double ub, double dt, double L)
 {
     if (sg.form == 0) return ua + dt * L;                          // U + dt L            (Eq.6/7 first line)
@@ -409,14 +378,14 @@ int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua,
 // FORM (the RK form of the stage) and CFL (last stage of a step) are compile-time: the stage loop has no form branches, and the
 // signal-speed code with its block reduction exists only in the instantiations that need it.
 template <int EK, int FORM, bool CFL>
-__global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
+__global__ void __launch_bounds__(XT, 768 / XT) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
                                                           Source src, StepState* ds)
 {
-    __shared__ double sF[5][TPB];
+    __shared__ double sF[5][XT];
     const int t = threadIdx.x;
     const int nf = g.n[0] + 1;                                              // x interfaces per row
     const long long nrows = (long long)g.n[1] * g.n[2];
-    const long long I = (long long)blockIdx.x * (TPB - 1) + t;
+    const long long I = (long long)blockIdx.x * (XT - 1) + t;
     const bool live = I < nrows * nf;
     int f = 0, j = 0, kz = 0;
     unsigned int p = 0;                                                      // cell offsets fit 32 bits (mf_create)
@@ -434,7 +403,7 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
 #pragma unroll
         for (int v = 0; v < 5; ++v) { A[v] = fc.f[0][1][v][p] + fc.f[0][0][v][p]; B[v] = fc.f[0][1][v][p + 1] - fc.f[0][0][v][p + 1]; }
 #endif
-        if (t < TPB - 1 && f < g.n[0]) {                                    // pull the combine's operands towards L2 while MUSTA runs
+        if (t < XT - 1 && f < g.n[0]) {                                    // pull the combine's operands towards L2 while MUSTA runs
             const unsigned int pc = p + 1, o = eo + f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
 #pragma unroll
             for (int v = 0; v < 5; ++v) {
@@ -451,7 +420,7 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
     __syncthreads();
     double smax = 0.0;
     int bad = 0;
-    if (live && t < TPB - 1 && f < g.n[0]) {                                // cell (f, j, kz): lower x face = this interface, upper = thread t+1's
+    if (live && t < XT - 1 && f < g.n[0]) {                                // cell (f, j, kz): lower x face = this interface, upper = thread t+1's
         const unsigned int pc = p + 1;
         const unsigned int o = eo + f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
         const double dt = ds->dt;
@@ -476,15 +445,15 @@ __global__ void __launch_bounds__(TPB, 3) k_xflux_combine(Grid g, Eos q, int k, 
         }
         if (CFL) smax = signal_speed<EK>(q, W[0], W[1], W[2], W[3], W[4], bad);
     }
-    if (CFL) block_reduce_smax(smax, bad, ds);
+    if (CFL) block_reduce_smax<XT>(smax, bad, ds);
 }
 
 int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src,
                          StepState* ds, cudaStream_t st)
 {
     const long long total = (long long)(g.n[0] + 1) * g.n[1] * g.n[2];
-    const dim3 nb(blocks_for(total, TPB - 1), g.nev);
-#define MF_XFC(EK_, FORM_, CFL_) k_xflux_combine<EK_, FORM_, CFL_><<<nb, TPB, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds)
+    const dim3 nb(blocks_for(total, XT - 1), g.nev);
+#define MF_XFC(EK_, FORM_, CFL_) k_xflux_combine<EK_, FORM_, CFL_><<<nb, XT, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds)
 #define MF_XFC_FORMS(EK_) \
     if (sg.form == 0) { if (sg.cfl) MF_XFC(EK_, 0, true); else MF_XFC(EK_, 0, false); } \
     else if (sg.form == 1) { if (sg.cfl) MF_XFC(EK_, 1, true); else MF_XFC(EK_, 1, false); } \

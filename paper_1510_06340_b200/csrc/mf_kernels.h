@@ -33,6 +33,13 @@ int launch_tile_stage(const Grid& g, const Eos& q, int limiter, int predictor, i
 int launch_tile_stage_pre(const Grid& g, const Eos& q, int k, Faces fc, CState5 V, Stage sg, CState5 Ua, State5 out, Source src,
                           const StepState* ds, int num_sms, cudaStream_t st);
 
+// ---- sweep path (MF_PATH_SWEEP, mf_sweep.cu): per-direction sweeps that limit the slopes themselves from a +-2-cell halo of V; with pred the
+// Hancock increment Dl (extended layout, from launch_delta_stage) is added to both face states.  F_y, F_z go to fx, the x sweep finishes the cells.
+bool sweep_supported(const Grid& g, int eos_kind, int predictor);
+int launch_sweep_flux(const Grid& g, const Eos& q, int limiter, int k, bool pred, CState5 V, CState5 Dl, Fluxes fx, const StepState* ds, cudaStream_t st);
+int launch_sweep_xcombine(const Grid& g, const Eos& q, int limiter, int k, bool pred, CState5 V, CState5 Dl, Fluxes fx, Stage sg, CState5 Ua, State5 out,
+                          Source src, StepState* ds, cudaStream_t st);
+
 // ---- conversions and reductions
 int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st);          // in place: (e,v,n) -> (E,M,R), Eq.4
 int launch_con2prim(const Grid& g, const Eos& q, CState5 U, State5 P, cudaStream_t st); // Eq.23
