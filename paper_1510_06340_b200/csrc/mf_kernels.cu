@@ -106,7 +106,7 @@ int launch_reset(StepState* ds, int nev, cudaStream_t st) { k_reset<<<(nev + 63)
 // =========================================================================== a3 + a4: cell stage
 // One thread per cell of the extended region (interior + 1 layer on every active axis).
 template <int LIM, int EK>
-__global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, int predictor, CState5 V, Faces fc, const StepState* ds)
+__global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, int predictor, CState5 V, Faces fc, State5 Wout, const StepState* ds)
 {
     // linear index over the extended region, x fastest: 256 consecutive cells per block (measured on B200: 32 x 8 tiles, which
     // reuse the y neighbours through L1, are 10-15% slower because the DRAM bursts get shorter)
@@ -237,18 +237,19 @@ __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, 
 #pragma unroll
         for (int v = 0; v < 5; ++v) W[v] = fma(hl, acc[v], U0[v]);
     }
-    const int dW = g.act[0] ? 0 : (g.act[1] ? 1 : 2);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) fc.f[dW][1][v][pu] = W[v];
+    for (int v = 0; v < 5; ++v) Wout.q[v][pu] = W[v];                        // = fc.f[first active axis][1]
 #endif
 }
 
 int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, CState5 V, Faces fc, const StepState* ds, cudaStream_t st)
 {
     const dim3 nb(blocks_for(g.next, CT), g.nev);
+    State5 Wout;
+    for (int v = 0; v < 5; ++v) Wout.q[v] = fc.f[g.act[0] ? 0 : (g.act[1] ? 1 : 2)][1][v];
     switch (limiter) {
-#define MF_CASE(L) case L: if (q.kind) k_cell_stage<L, 1><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, ds); \
-                           else k_cell_stage<L, 0><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, ds); break;
+#define MF_CASE(L) case L: if (q.kind) k_cell_stage<L, 1><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); \
+                           else k_cell_stage<L, 0><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); break;
         MF_CASE(LIM_NONE) MF_CASE(LIM_MINMOD) MF_CASE(LIM_SUPERBEE) MF_CASE(LIM_VANALBADA) MF_CASE(LIM_VANLEER) MF_CASE(LIM_MC) MF_CASE(LIM_FIRST)
 #undef MF_CASE
     default: return 0;
@@ -259,7 +260,7 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
 // =========================================================================== a5 + a6: interface fluxes
 // One thread per interface between cell c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
 template <int D, int EK>
-__global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, int k, Faces fc, Fluxes fx, const StepState* ds)
+__global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, int k, CState5 Wc, Faces fc, Fluxes fx, const StepState* ds)
 {
     int m[3] = { g.n[0], g.n[1], g.n[2] };
     m[D] += 1;
@@ -278,10 +279,9 @@ __global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, 
     for (int v = 0; v < 5; ++v) { A[v] = fc.f[D][1][v][p]; B[v] = fc.f[D][0][v][p + es[D]]; }   // A2 :173
 #else
     {                                                                                             // compact scratch: W and H_D
-        const int dW = g.act[0] ? 0 : (g.act[1] ? 1 : 2);
-        const unsigned int pn = p + es[D];
-#pragma unroll
-        for (int v = 0; v < 5; ++v) { A[v] = fc.f[dW][1][v][p] + fc.f[D][0][v][p]; B[v] = fc.f[dW][1][v][pn] - fc.f[D][0][v][pn]; }
+        const unsigned int pn = p + es[D];                          // (W's arrays come as an argument of their own: picking them out of fc
+#pragma unroll                                                      //  with a runtime index costs indexed constant loads the loads then wait for)
+        for (int v = 0; v < 5; ++v) { A[v] = Wc.q[v][p] + fc.f[D][0][v][p]; B[v] = Wc.q[v][pn] - fc.f[D][0][v][pn]; }
     }
 #endif
     musta_flux<D, EK>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
@@ -292,14 +292,16 @@ __global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, 
 int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, Fluxes fx, const StepState* ds, cudaStream_t st)
 {
     int launches = 0;
+    CState5 Wc;
+    for (int v = 0; v < 5; ++v) Wc.q[v] = fc.f[g.act[0] ? 0 : (g.act[1] ? 1 : 2)][1][v];
     for (int d = 0; d < 3; ++d) {
         if (!g.act[d] || !(dmask & (1 << d))) continue;
         long long total = 1;
         for (int a = 0; a < 3; ++a) total *= (a == d) ? g.n[a] + 1 : g.n[a];
         const dim3 nb(blocks_for(total, FT), g.nev);
-        if (d == 0) { if (q.kind) k_flux_stage<0, 1><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<0, 0><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); }
-        if (d == 1) { if (q.kind) k_flux_stage<1, 1><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<1, 0><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); }
-        if (d == 2) { if (q.kind) k_flux_stage<2, 1><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); else k_flux_stage<2, 0><<<nb, FT, 0, st>>>(g, q, k, fc, fx, ds); }
+        if (d == 0) { if (q.kind) k_flux_stage<0, 1><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); else k_flux_stage<0, 0><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); }
+        if (d == 1) { if (q.kind) k_flux_stage<1, 1><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); else k_flux_stage<1, 0><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); }
+        if (d == 2) { if (q.kind) k_flux_stage<2, 1><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); else k_flux_stage<2, 0><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); }
         ++launches;
     }
     return launches;
