@@ -87,9 +87,11 @@ def alg_bytes(rk):
     return 80 + 120 * (rk - 1) + 32
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch group at 256^3 (config 3, staged path), one ncu --set full capture:
-# k_cell_stage 3.393 GB; k_flux_stage<1>, <2> 2.033 + 2.038 GB; k_xflux_combine 4.721 GB (profiles/r01_ncu_full_staged_256.md)
-NCU_TRAFFIC_GB_256 = {"cell_stage": 3.393, "flux_stage": 4.071, "combine": 4.721}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch group at 256^3 (config 3 scheme), one ncu --set full capture per path:
+# staged: k_cell_stage 3.375 GB; k_flux_stage<1>, <2> 2.031 + 2.032 GB; k_xflux_combine 4.721 GB (profiles/r01_ncu_full_staged_256.md)
+# sweep (predictor off): k_sweep_flux<1>, <2> 1.328 + 1.339 GB; k_sweep_xcombine 3.361 GB (profiles/r01_ncu_full_sweep_256.md)
+NCU_TRAFFIC_GB_256 = {("staged", True): {"cell_stage": 3.375, "flux_stage": 4.063, "combine": 4.721},
+                      ("sweep", False): {"flux_stage": 2.667, "combine": 3.361}}
 
 FP64_LANES_PER_SM = 64       # B200 (sm_100): 4 SMSPs x 16 FP64 lanes; mf_probe_fp64 measures it
 
@@ -355,9 +357,9 @@ def run_ours(args):
         kernels[name] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak, "traffic": None,
                          "kernel": name, "launch_ms": ms / groups, "share_of_step": ms / elapsed_ms,
                          "alg_slots_per_cell": slots, "alg_bytes_per_cell": nbytes}
-    # DRAM traffic per launch group from the committed ncu --set full capture of this same workload (profiles/r01_ncu_full_staged_256.md)
-    if g.path() == "staged" and (nx, ny, nz) == (256, 256, 256) and sch["k_stages"] == 3 and sch["rk"] == 3:
-        for name, gb in NCU_TRAFFIC_GB_256.items():
+    # DRAM traffic per launch group from the committed ncu --set full capture of this same workload and path (profiles/r01_ncu_full_*_256.md)
+    if (nx, ny, nz) == (256, 256, 256) and sch["k_stages"] == 3 and sch["rk"] == 3 and nbatch == 1 and args.eos == "cs2":
+        for name, gb in NCU_TRAFFIC_GB_256.get((g.path(), bool(pred_on)), {}).items():
             if name in kernels:
                 kernels[name]["traffic"] = gb * 1e9
     # the dominant kernel class = the one with the largest share of the timed region
