@@ -118,6 +118,13 @@ int mf_set_alpha(mf_ctx*, double alpha);    /* FORCE alpha, default = number of 
 int mf_set_jet_source(mf_ctx*, double dEdx, double sigma, double x0, double y0, double z0);
 int mf_set_path(mf_ctx*, int path);         /* MF_PATH_*; MF_EINVAL if that path cannot run this configuration */
 int mf_get_path(mf_ctx*, int* path);        /* the path mf_step will actually take */
+/* Low-storage Runge-Kutta (:117 "a low storage version of the third order method can be used"; the paper prints no formula): the same
+ * Eq.6 / Eq.7 arithmetic with two state registers instead of three - every stage after the first replaces the work register in place, so
+ * the results are bit-identical to the three-register form.  Frees (on = 1) or re-allocates (on = 0) the third register; synchronises.
+ * Staged path only (MF_PATH_AUTO then resolves to it); MF_EINVAL if another path is selected. */
+int mf_set_low_storage(mf_ctx*, int on);
+/* Device memory currently held by the context (state registers, scratch allocated so far, tables), in bytes. */
+int mf_memory_bytes(mf_ctx*, long long* bytes);
 /* Run on a caller-owned CUDA stream (a cudaStream_t passed as void*), e.g. PyTorch's current stream, so the
  * caller's events bracket the kernels.  NULL restores the context's own stream. */
 int mf_set_stream(mf_ctx*, void* cuda_stream);

@@ -50,6 +50,8 @@ SIGNATURES = {
     "mf_set_jet_source": (C.c_int, [_vp] + [C.c_double] * 5),
     "mf_set_path": (C.c_int, [_vp, C.c_int]),
     "mf_get_path": (C.c_int, [_vp, C.POINTER(C.c_int)]),
+    "mf_set_low_storage": (C.c_int, [_vp, C.c_int]),
+    "mf_memory_bytes": (C.c_int, [_vp, C.POINTER(C.c_longlong)]),
     "mf_set_stream": (C.c_int, [_vp, _vp]),
     "mf_sync": (C.c_int, [_vp]),
     "mf_last_error": (C.c_char_p, [_vp]),
@@ -231,6 +233,14 @@ class MustaForce:
 
     def set_path(self, path):
         self._chk(self.lib.mf_set_path(self.h, PATH[path] if isinstance(path, str) else int(path)))
+
+    def set_low_storage(self, on):
+        self._chk(self.lib.mf_set_low_storage(self.h, 1 if on else 0))
+
+    def memory_bytes(self):
+        b = C.c_longlong()
+        self._chk(self.lib.mf_memory_bytes(self.h, C.byref(b)))
+        return b.value
 
     def path(self):
         p = C.c_int()

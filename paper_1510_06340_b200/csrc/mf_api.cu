@@ -31,6 +31,7 @@ struct mf_ctx {
     int nev;                 // events in the batch (1 unless mf_create_batch)
     long long nst, nxt;      // nev*ncell, nev*next: the length of one component array in the interior / extended layout
     double* U[3];            // three state registers, 5*nst doubles each (U^n, U_(1), U_(2)), component-major, [component][event][cell]
+    int nreg;                // 3, or 2 in low-storage mode (mf_set_low_storage): U[2] is then not allocated
     int cur;                 // which register holds U^n
     double* faces;           // staged path: 2*5*nact*next doubles
     double* fluxes;          // staged path: 5*nact*next doubles
@@ -110,6 +111,13 @@ void clear_table(Eos& q)
 
 int resolve_path(mf_ctx* c)
 {
+    if (c->nreg == 2) {
+        // low storage: an RK stage writes its result over the register it read, which only the staged path's last kernel allows (it touches
+        // the state at the thread's own cell only; the sweep and tile kernels read neighbours of the state they are replacing)
+        if (c->path_req != MF_PATH_AUTO && c->path_req != MF_PATH_STAGED) return MF_EINVAL;
+        c->path = MF_PATH_STAGED;
+        return MF_OK;
+    }
     if (c->path_req == MF_PATH_FUSED || c->path_req == MF_PATH_HYBRID) {
         if (!fused_supported(c->g) || c->eos != MF_EOS_CS2 || c->nev > 1) return MF_EINVAL;      // the tile kernel is built for p = cs2*e and three active axes
         c->path = c->path_req;
@@ -257,9 +265,31 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
 int run_step(mf_ctx* c)
 {
     double* Un = c->U[c->cur];
+    int rc;
+    if (c->nreg == 2) {
+        // Low-storage form (:117): the same Eq.6 / Eq.7 arithmetic with ONE work register next to U^n; stages 2 and 3 replace the work
+        // register in place (the x kernel reads U_(s) at its own cell before it stores there).
+        double* Rw = c->U[1 - c->cur];
+        Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
+        if ((rc = run_stage(c, Un, s1, Un, Rw)) != MF_OK) return rc;
+        if (c->rk == 2) {
+            Stage s2 = { 1, 0.5, 0.5, 1.0, 1.0 };
+            s2.cfl = 1;
+            if ((rc = run_stage(c, Rw, s2, Un, Rw)) != MF_OK) return rc;
+        } else {
+            Stage s2 = { 2, 0.75, 0.25, 0.25, 1.0 };
+            Stage s3 = { 2, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, 0.5 };
+            s3.cfl = 1;
+            if ((rc = run_stage(c, Rw, s2, Un, Rw)) != MF_OK) return rc;
+            if ((rc = run_stage(c, Rw, s3, Un, Rw)) != MF_OK) return rc;
+        }
+        c->cur = 1 - c->cur;
+        c->launches += launch_end_step(c->ds, c->nev, c->stream);
+        c->smax_valid = 1;
+        return MF_OK;
+    }
     double* Ra = c->U[(c->cur + 1) % 3];
     double* Rb = c->U[(c->cur + 2) % 3];
-    int rc;
     if (c->rk == 2) {
         Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
         Stage s2 = { 1, 0.5, 0.5, 1.0, 1.0 };
@@ -369,7 +399,7 @@ mf_ctx* mf_create_batch(int nevents, int nx, int ny, int nz, double dx, int eos,
     c->limiter = limiter; c->k = k_stages; c->rk = 2; c->predictor = 1;
     c->alpha = c->nact > 0 ? (double)c->nact : 1.0;                 // A9
     memset(&c->src, 0, sizeof(c->src));
-    c->path_req = MF_PATH_AUTO; c->cur = 0; c->launches = 0;
+    c->path_req = MF_PATH_AUTO; c->cur = 0; c->nreg = 3; c->launches = 0;
     c->prof_on = 0; c->prof_used = 0; c->smax_valid = 0;
     resolve_path(c);
     c->nblocks_tot = c->num_sms * 4;
@@ -556,7 +586,7 @@ int mf_get_state_prim(mf_ctx* c, double* e, double* vx, double* vy, double* vz, 
 {
     if (!c) return MF_EINVAL;
     if (!e || !vx || !vy || !vz || !n) return fail(c, MF_EINVAL, "null pointer");
-    double* scratch = c->U[(c->cur + 1) % 3];
+    double* scratch = c->U[(c->cur + 1) % c->nreg];
     c->launches += launch_con2prim(c->g, c->q, cstate(c->U[c->cur], c->nst), state(scratch, c->nst), c->stream);
     int rc = check_launch(c);
     if (rc != MF_OK) return rc;
@@ -599,7 +629,7 @@ int mf_eval_L(mf_ctx* c, double dt, double* L_E, double* L_Mx, double* L_My, dou
     if (!c) return MF_EINVAL;
     if (!(dt > 0.0) || !L_E || !L_Mx || !L_My || !L_Mz || !L_R) return fail(c, MF_EINVAL, "bad dt or null pointer");
     double* Un = c->U[c->cur];
-    double* scratch = c->U[(c->cur + 1) % 3];
+    double* scratch = c->U[(c->cur + 1) % c->nreg];
     c->launches += launch_begin_step(c->ds, c->nev, 1, dt, c->g.dx, c->alpha, c->stream);
     Stage sg = { 3, 0.0, 0.0, 0.0, 0.0 };
     c->smax_valid = 0;
@@ -754,9 +784,44 @@ int mf_set_path(mf_ctx* c, int path)
     if (path < MF_PATH_AUTO || path > MF_PATH_SWEEP) return fail(c, MF_EINVAL, "unknown path");
     int keep = c->path_req;
     c->path_req = path;
-    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "this path does not support this configuration (fused/hybrid: three active axes, MF_EOS_CS2, one event; sweep: active x axis, MF_EOS_CS2, and with the predictor on a 3D grid and one event)"); }
+    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "this path does not support this configuration (fused/hybrid: three active axes, MF_EOS_CS2, one event; sweep: active x axis, MF_EOS_CS2, and with the predictor on a 3D grid and one event; low storage: staged only)"); }
     return MF_OK;
 }
+int mf_set_low_storage(mf_ctx* c, int on)
+{
+    if (!c) return MF_EINVAL;
+    on = on ? 1 : 0;
+    if (on == (c->nreg == 2)) return MF_OK;
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (on) {
+        c->nreg = 2;
+        if (resolve_path(c) != MF_OK) { c->nreg = 3; resolve_path(c); return fail(c, MF_EINVAL, "low-storage Runge-Kutta runs on the staged path only: select MF_PATH_AUTO or MF_PATH_STAGED first"); }
+        if (c->cur == 2) {                                         // bring U^n into one of the two registers that stay
+            MF_CUDA(c, cudaMemcpy(c->U[0], c->U[2], sizeof(double) * 5 * c->nst, cudaMemcpyDeviceToDevice));
+            c->cur = 0;
+        }
+        cudaFree(c->U[2]); c->U[2] = nullptr;
+    } else {
+        if (cudaMalloc(&c->U[2], sizeof(double) * 5 * c->nst) != cudaSuccess) { cudaGetLastError(); c->U[2] = nullptr; return fail(c, MF_ENOMEM, "cudaMalloc(third state register) failed"); }
+        c->nreg = 3;
+        resolve_path(c);
+    }
+    return MF_OK;
+}
+
+int mf_memory_bytes(mf_ctx* c, long long* bytes)
+{
+    if (!c || !bytes) return MF_EINVAL;
+    long long b = (long long)sizeof(double) * 5 * c->nst * c->nreg;
+    if (c->faces) b += (long long)sizeof(double) * 10 * c->nact * c->nxt;
+    if (c->fluxes) b += (long long)sizeof(double) * 5 * c->nact * c->nxt;
+    if (c->delta) b += (long long)sizeof(double) * 5 * c->g.next;
+    if (c->table) b += (long long)(sizeof(double) + sizeof(float)) * c->q.ne * c->q.nn;
+    b += (long long)sizeof(StepState) * c->nev + (long long)sizeof(double) * 5 * c->nblocks_tot;
+    *bytes = b;
+    return MF_OK;
+}
+
 int mf_get_path(mf_ctx* c, int* path) { if (!c || !path) return MF_EINVAL; *path = c->path; return MF_OK; }
 
 } // extern "C"

@@ -275,3 +275,46 @@ def test_full_size_config5_512_window_with_jet():
     jx = int(round((st["jet"]["x0"]) / st["dx"] + nx / 2.0))
     r = _windowed_parity(st, (nz // 2, ny // 2, jx), steps_before=2, m=1, half=8)
     print("512^3 window", r)
+
+
+# ------------------------------------------------------------------ low-storage Runge-Kutta
+@pytest.mark.parametrize("rk,limiter,k,predictor", [(3, "superbee", 3, True), (2, "mc", 2, True), (3, "minmod", 2, False)])
+def test_low_storage_rk_is_bit_identical_and_smaller(rk, limiter, k, predictor):
+    """Two state registers instead of three, the same Eq.6 / Eq.7 arithmetic: the bits must not change, the footprint must."""
+    st = w.lumpy_event(shape=(20, 24, 28), dx=0.2, n_gauss=6, radius=1.5, half_z=1.0, background=0.5)
+    kw = dict(dx=0.2, limiter=limiter, k_stages=k, rk=rk, bc="outflow", predictor=predictor)
+    out, mem = {}, {}
+    for low in (False, True):
+        g = MustaForce(28, 24, 20, path="staged", **kw)
+        g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+        g.step(2, 0.3)                                                # cur has moved off register 0 before the switch
+        if low:
+            g.set_low_storage(True)
+        g.step(9, 0.3)
+        g.step_dt(2, 0.01)
+        out[low], mem[low] = g.get_state(), g.memory_bytes()
+        prim = g.get_state_prim()                                     # uses the free register as scratch
+        assert all(np.all(np.isfinite(a)) for a in prim)
+        assert g.path() == "staged"
+    for a, b in zip(out[True], out[False]):
+        assert np.array_equal(a, b)
+    n = 28 * 24 * 20
+    assert mem[False] - mem[True] == 40 * n
+    o = parity.make_pair(st, **{k_: v for k_, v in kw.items() if k_ != "dx"})[1]
+    o.step(11, 0.3)
+    o.step_dt(2, 0.01)
+    parity.assert_parity(out[True], o.get_state(), what="low-storage RK%d against the oracle" % rk)
+
+
+def test_low_storage_path_rules():
+    g = MustaForce(16, 16, 16, dx=0.1, predictor=False)
+    assert g.path() == "sweep"
+    g.set_low_storage(True)                                            # AUTO falls back to the staged path, the only one that may write in place
+    assert g.path() == "staged"
+    with pytest.raises(MustaForceError):
+        g.set_path("sweep")
+    g.set_low_storage(False)
+    assert g.path() == "sweep"
+    h = MustaForce(16, 16, 16, dx=0.1, path="fused")
+    with pytest.raises(MustaForceError):
+        h.set_low_storage(True)
