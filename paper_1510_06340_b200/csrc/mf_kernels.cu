@@ -16,6 +16,9 @@ namespace mf {
 #ifndef MF_XC_TPB
 #define MF_XC_TPB 128
 #endif
+#ifndef MF_XC_MINB
+#define MF_XC_MINB 5        // x kernel: 5 blocks of 128 threads (96 registers): the combine holds its 30 operands in registers at once
+#endif
 #ifndef MF_CELL_MINB
 #define MF_CELL_MINB (768 / MF_CELL_TPB)
 #endif
@@ -332,6 +335,17 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
         const double dt = ds->dt;
         double S = 0.0;
         if (src.on) S = jet_source(g, src, i, j, k, ds->t + sg.ts * dt);
+        double fhi[3][5], flo[3][5], ua5[5], ub5[5];                   // all loads before the first store (see k_xflux_combine)
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                if (!g.act[d]) continue;
+                fhi[d][v] = fx.f[d][v][p]; flo[d][v] = fx.f[d][v][p - (unsigned int)g.es[d]];
+            }
+            ua5[v] = sg.form == 3 ? 0.0 : Ua.q[v][o];
+            ub5[v] = (sg.form == 1 || sg.form == 2) ? Ub.q[v][o] : 0.0;
+        }
         double W[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
@@ -340,7 +354,7 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 if (!g.act[d]) continue;
-                double diff = fx.f[d][v][p] - fx.f[d][v][p - (unsigned int)g.es[d]];
+                double diff = fhi[d][v] - flo[d][v];
                 acc = first ? diff : acc + diff;
                 first = false;
             }
@@ -350,9 +364,7 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
             double L = -acc * g.inv_dx;
 #endif
             if (src.on && v < 2) L = L + S;
-            double ua = sg.form == 3 ? 0.0 : Ua.q[v][o];
-            double ub = (sg.form == 1 || sg.form == 2) ? Ub.q[v][o] : 0.0;
-            W[v] = rk_form(sg, ua, ub, dt, L);
+            W[v] = rk_form(sg, ua5[v], ub5[v], dt, L);
             out.q[v][o] = W[v];
         }
         if (sg.cfl) smax = signal_speed<EK>(q, W[0], W[1], W[2], W[3], W[4], bad);   // a2 for the next step, while U^{n+1} is in registers
@@ -380,7 +392,7 @@ int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua,
 // FORM (the RK form of the stage) and CFL (last stage of a step) are compile-time: the stage loop has no form branches, and the
 // signal-speed code with its block reduction exists only in the instantiations that need it.
 template <int EK, int FORM, bool CFL>
-__global__ void __launch_bounds__(XT, 768 / XT) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
+__global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
                                                           Source src, StepState* ds)
 {
     __shared__ double sF[5][XT];
@@ -428,20 +440,29 @@ __global__ void __launch_bounds__(XT, 768 / XT) k_xflux_combine(Grid g, Eos q, i
         const double dt = ds->dt;
         double S = 0.0;
         if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
+        // every operand is loaded before the first store: `out` may alias the inputs as far as the compiler knows (and does alias U_(s) in
+        // low-storage mode), so loads written after a store would wait for it - five dependent round trips to memory instead of one
+        double fy1[5], fy0[5], fz1[5], fz0[5], ua5[5], ub5[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+            if (g.act[1]) { fy1[v] = fx.f[1][v][pc]; fy0[v] = fx.f[1][v][pc - (unsigned int)g.es[1]]; }
+            if (g.act[2]) { fz1[v] = fx.f[2][v][pc]; fz0[v] = fx.f[2][v][pc - (unsigned int)g.es[2]]; }
+            ua5[v] = FORM == 3 ? 0.0 : Ua.q[v][o];
+            ub5[v] = (FORM == 1 || FORM == 2) ? Ub.q[v][o] : 0.0;
+        }
         double W[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
             double acc = sF[v][t + 1] - F[v];
-            if (g.act[1]) acc = acc + (fx.f[1][v][pc] - fx.f[1][v][pc - (unsigned int)g.es[1]]);
-            if (g.act[2]) acc = acc + (fx.f[2][v][pc] - fx.f[2][v][pc - (unsigned int)g.es[2]]);
+            if (g.act[1]) acc = acc + (fy1[v] - fy0[v]);
+            if (g.act[2]) acc = acc + (fz1[v] - fz0[v]);
 #ifdef MF_STRICT
             double L = -acc / g.dx;                                        // Eq.1 :43
 #else
             double L = -acc * g.inv_dx;
 #endif
             if (src.on && v < 2) L = L + S;
-            const double ua = FORM == 3 ? 0.0 : Ua.q[v][o];
-            const double ub = (FORM == 1 || FORM == 2) ? Ub.q[v][o] : 0.0;
+            const double ua = ua5[v], ub = ub5[v];
             W[v] = FORM == 0 ? ua + dt * L : (FORM == 1 ? 0.5 * (ua + ub + dt * L) : (FORM == 2 ? sg.ca * ua + sg.cb * ub + (sg.cdt * dt) * L : L));
             out.q[v][o] = W[v];
         }

@@ -107,7 +107,10 @@ __global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, i
 #ifndef MF_XT
 #define MF_XT 128
 #endif
-constexpr int XT = MF_XT, XB = 768 / MF_XT;      // threads per block of the x sweep, blocks per SM (24 warps at 80 registers)
+#ifndef MF_XB
+#define MF_XB 6
+#endif
+constexpr int XT = MF_XT, XB = MF_XB;                // threads per block of the x sweep, blocks per SM (measured: 6 x 128 at 80 registers beats 5 x 128 at 96 here)
 template <bool PRED, int FORM, bool CFL>
 __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int lim, int k, CState5 V, CState5 Dl, Fluxes fx, Stage sg, CState5 Ua,
                                                            State5 out, Source src, StepState* ds)
@@ -162,20 +165,29 @@ __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int li
         const double dt = ds->dt;
         double S = 0.0;
         if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
+        // every operand is loaded before the first store (`out` may alias the inputs as far as the compiler knows: loads written after a
+        // store would wait for it - five dependent round trips to memory instead of one)
+        double fy1[5], fy0[5], fz1[5], fz0[5], ua5[5], ub5[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+            if (g.act[1]) { fy1[v] = fx.f[1][v][pc]; fy0[v] = fx.f[1][v][pc - (unsigned int)g.es[1]]; }
+            if (g.act[2]) { fz1[v] = fx.f[2][v][pc]; fz0[v] = fx.f[2][v][pc - (unsigned int)g.es[2]]; }
+            ua5[v] = FORM == 3 ? 0.0 : Ua.q[v][oc];
+            ub5[v] = (FORM == 1 || FORM == 2) ? V.q[v][oc] : 0.0;           // U_(s) is the state the sweep ran on
+        }
         double W[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
             double acc = sF[v][t + 1] - F[v];
-            if (g.act[1]) acc = acc + (fx.f[1][v][pc] - fx.f[1][v][pc - (unsigned int)g.es[1]]);
-            if (g.act[2]) acc = acc + (fx.f[2][v][pc] - fx.f[2][v][pc - (unsigned int)g.es[2]]);
+            if (g.act[1]) acc = acc + (fy1[v] - fy0[v]);
+            if (g.act[2]) acc = acc + (fz1[v] - fz0[v]);
 #ifdef MF_STRICT
             double L = -acc / g.dx;                                        // Eq.1 :43
 #else
             double L = -acc * g.inv_dx;
 #endif
             if (src.on && v < 2) L = L + S;
-            const double ua = FORM == 3 ? 0.0 : Ua.q[v][oc];
-            const double ub = (FORM == 1 || FORM == 2) ? V.q[v][oc] : 0.0;  // U_(s) is the state the sweep ran on
+            const double ua = ua5[v], ub = ub5[v];
             W[v] = FORM == 0 ? ua + dt * L : (FORM == 1 ? 0.5 * (ua + ub + dt * L) : (FORM == 2 ? sg.ca * ua + sg.cb * ub + (sg.cdt * dt) * L : L));
             out.q[v][oc] = W[v];
         }
