@@ -19,6 +19,9 @@ namespace mf {
 #ifndef MF_XC_MINB
 #define MF_XC_MINB 5        // x kernel: 5 blocks of 128 threads (96 registers): the combine holds its 30 operands in registers at once
 #endif
+#ifndef MF_CELL_PF
+#define MF_CELL_PF (148 * 768)   // cells ahead (in the plane above) whose lines a cell-stage thread prefetches to L2: one wave of resident threads; 0 = off
+#endif
 #ifndef MF_CELL_MINB
 #define MF_CELL_MINB (768 / MF_CELL_TPB)
 #endif
@@ -130,6 +133,17 @@ __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, 
     double U0[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) U0[v] = V.q[v][o0];
+#if MF_CELL_PF
+    // The kernel is latency bound, and the only lines a block meets for the first time are those of the plane above (z+1): everything else
+    // was touched by the blocks before it.  Pull that plane's lines for the cells one wave of blocks ahead towards L2.
+    if (g.act[2]) {
+        const unsigned int opf = o0 + ns[2] + (unsigned int)MF_CELL_PF;
+        if (opf < (blockIdx.y + 1u) * (unsigned int)g.ncell) {
+#pragma unroll
+            for (int v = 0; v < 5; ++v) prefetch_l2(&V.q[v][opf]);
+        }
+    }
+#endif
 
 #ifdef MF_STRICT
     double UL[3][5], UR[3][5];
