@@ -443,20 +443,14 @@ __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q,
         }
         musta_flux<0, EK>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
     }
-#pragma unroll
-    for (int v = 0; v < 5; ++v) sF[v][t] = F[v];
-    __syncthreads();
-    double smax = 0.0;
-    int bad = 0;
-    if (live && t < XT - 1 && f < g.n[0]) {                                // cell (f, j, kz): lower x face = this interface, upper = thread t+1's
-        const unsigned int pc = p + 1;
-        const unsigned int o = eo + f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
-        const double dt = ds->dt;
-        double S = 0.0;
-        if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
-        // every operand is loaded before the first store: `out` may alias the inputs as far as the compiler knows (and does alias U_(s) in
-        // low-storage mode), so loads written after a store would wait for it - five dependent round trips to memory instead of one
-        double fy1[5], fy0[5], fz1[5], fz0[5], ua5[5], ub5[5];
+    // The combine's operands.  Every one is loaded before the first store: `out` may alias the inputs as far as the compiler knows (and does
+    // alias U_(s) in low-storage mode), so loads written after a store would wait for it - five dependent round trips to memory instead of
+    // one.  And they are issued BEFORE the barrier, so that their latency runs while the block's other warps finish MUSTA.
+    const bool owns_cell = live && t < XT - 1 && f < g.n[0];                // cell (f, j, kz): lower x face = this interface, upper = thread t+1's
+    const unsigned int pc = p + 1;
+    const unsigned int o = eo + f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
+    double fy1[5], fy0[5], fz1[5], fz0[5], ua5[5], ub5[5];
+    if (owns_cell) {
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
             if (g.act[1]) { fy1[v] = fx.f[1][v][pc]; fy0[v] = fx.f[1][v][pc - (unsigned int)g.es[1]]; }
@@ -464,6 +458,16 @@ __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q,
             ua5[v] = FORM == 3 ? 0.0 : Ua.q[v][o];
             ub5[v] = (FORM == 1 || FORM == 2) ? Ub.q[v][o] : 0.0;
         }
+    }
+#pragma unroll
+    for (int v = 0; v < 5; ++v) sF[v][t] = F[v];
+    __syncthreads();
+    double smax = 0.0;
+    int bad = 0;
+    if (owns_cell) {
+        const double dt = ds->dt;
+        double S = 0.0;
+        if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
         double W[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {

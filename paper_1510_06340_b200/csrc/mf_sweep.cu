@@ -108,9 +108,9 @@ __global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, i
 #define MF_XT 128
 #endif
 #ifndef MF_XB
-#define MF_XB 6
+#define MF_XB 5
 #endif
-constexpr int XT = MF_XT, XB = MF_XB;                // threads per block of the x sweep, blocks per SM (measured: 6 x 128 at 80 registers beats 5 x 128 at 96 here)
+constexpr int XT = MF_XT, XB = MF_XB;                // threads per block of the x sweep, blocks per SM (96 registers: the combine holds its operands across the barrier)
 template <bool PRED, int FORM, bool CFL>
 __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int lim, int k, CState5 V, CState5 Dl, Fluxes fx, Stage sg, CState5 Ua,
                                                            State5 out, Source src, StepState* ds)
@@ -154,20 +154,14 @@ __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int li
         }
         musta_flux<0, 0>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
     }
-#pragma unroll
-    for (int v = 0; v < 5; ++v) sF[v][t] = F[v];
-    __syncthreads();
-    double smax = 0.0;
-    int bad = 0;
-    if (live && t < XT - 1 && f < g.n[0]) {                                // cell (f, j, kz): lower x face = this interface, upper = thread t+1's
-        const unsigned int pc = p + 1;
-        const unsigned int oc = row + f;
-        const double dt = ds->dt;
-        double S = 0.0;
-        if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
-        // every operand is loaded before the first store (`out` may alias the inputs as far as the compiler knows: loads written after a
-        // store would wait for it - five dependent round trips to memory instead of one)
-        double fy1[5], fy0[5], fz1[5], fz0[5], ua5[5], ub5[5];
+    // The combine's operands: all loaded before the first store (`out` may alias the inputs as far as the compiler knows: loads written after
+    // a store would wait for it - five dependent round trips to memory instead of one), and issued before the barrier, so that their
+    // latency runs while the block's other warps finish MUSTA.
+    const bool owns_cell = live && t < XT - 1 && f < g.n[0];                // cell (f, j, kz): lower x face = this interface, upper = thread t+1's
+    const unsigned int pc = p + 1;
+    const unsigned int oc = row + f;
+    double fy1[5], fy0[5], fz1[5], fz0[5], ua5[5], ub5[5];
+    if (owns_cell) {
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
             if (g.act[1]) { fy1[v] = fx.f[1][v][pc]; fy0[v] = fx.f[1][v][pc - (unsigned int)g.es[1]]; }
@@ -175,6 +169,16 @@ __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int li
             ua5[v] = FORM == 3 ? 0.0 : Ua.q[v][oc];
             ub5[v] = (FORM == 1 || FORM == 2) ? V.q[v][oc] : 0.0;           // U_(s) is the state the sweep ran on
         }
+    }
+#pragma unroll
+    for (int v = 0; v < 5; ++v) sF[v][t] = F[v];
+    __syncthreads();
+    double smax = 0.0;
+    int bad = 0;
+    if (owns_cell) {
+        const double dt = ds->dt;
+        double S = 0.0;
+        if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
         double W[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
