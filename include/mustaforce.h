@@ -123,6 +123,11 @@ int mf_get_path(mf_ctx*, int* path);        /* the path mf_step will actually ta
  * the results are bit-identical to the three-register form.  Frees (on = 1) or re-allocates (on = 0) the third register; synchronises.
  * Staged path only (MF_PATH_AUTO then resolves to it); MF_EINVAL if another path is selected. */
 int mf_set_low_storage(mf_ctx*, int on);
+/* mf_step / mf_step_dt replay whole steps from a CUDA graph when n >= 7 (5 in low-storage mode): one eager step, then one captured period of
+ * the register rotation (3 steps, or 2) launched repeatedly, the remainder eagerly.  The launches and their arguments are exactly the eager
+ * ones (every per-step scalar lives in device memory), so results are bit-identical; it removes the per-launch host cost that dominates
+ * small grids.  On by default; off while mf_profile is recording.  mf_set_graph(ctx, 0) forces eager launches. */
+int mf_set_graph(mf_ctx*, int on);
 /* Device memory currently held by the context (state registers, scratch allocated so far, tables), in bytes. */
 int mf_memory_bytes(mf_ctx*, long long* bytes);
 /* Run on a caller-owned CUDA stream (a cudaStream_t passed as void*), e.g. PyTorch's current stream, so the

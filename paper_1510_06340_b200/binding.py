@@ -51,6 +51,7 @@ SIGNATURES = {
     "mf_set_path": (C.c_int, [_vp, C.c_int]),
     "mf_get_path": (C.c_int, [_vp, C.POINTER(C.c_int)]),
     "mf_set_low_storage": (C.c_int, [_vp, C.c_int]),
+    "mf_set_graph": (C.c_int, [_vp, C.c_int]),
     "mf_memory_bytes": (C.c_int, [_vp, C.POINTER(C.c_longlong)]),
     "mf_set_stream": (C.c_int, [_vp, _vp]),
     "mf_sync": (C.c_int, [_vp]),
@@ -236,6 +237,9 @@ class MustaForce:
 
     def set_low_storage(self, on):
         self._chk(self.lib.mf_set_low_storage(self.h, 1 if on else 0))
+
+    def set_graph(self, on):
+        self._chk(self.lib.mf_set_graph(self.h, 1 if on else 0))
 
     def memory_bytes(self):
         b = C.c_longlong()

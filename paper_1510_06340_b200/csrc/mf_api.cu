@@ -47,6 +47,14 @@ struct mf_ctx {
     long long launches;
     std::string err;
     // per-class CUDA-event timing (mf_profile)
+    // CUDA-graph replay of whole steps (launch-bound grids): one captured period of the register rotation, keyed by what is baked into it
+    int graph_on;                          // mf_set_graph
+    unsigned long long epoch;              // bumped by every call that changes what a captured step would launch
+    cudaGraphExec_t graph_exec;
+    unsigned long long graph_epoch;
+    int graph_cur, graph_mode, graph_steps;
+    double graph_value;
+    long long graph_launches;
     int prof_on;
     std::vector<cudaEvent_t> prof_ev;     // pairs: [2i] start, [2i+1] stop
     std::vector<int> prof_cls;            // class of pair i
@@ -401,6 +409,8 @@ mf_ctx* mf_create_batch(int nevents, int nx, int ny, int nz, double dx, int eos,
     memset(&c->src, 0, sizeof(c->src));
     c->path_req = MF_PATH_AUTO; c->cur = 0; c->nreg = 3; c->launches = 0;
     c->prof_on = 0; c->prof_used = 0; c->smax_valid = 0;
+    c->graph_on = 1; c->epoch = 0; c->graph_exec = nullptr; c->graph_epoch = 0; c->graph_cur = -1; c->graph_mode = -1; c->graph_steps = 0;
+    c->graph_value = 0.0; c->graph_launches = 0;
     resolve_path(c);
     c->nblocks_tot = c->num_sms * 4;
 
@@ -438,6 +448,7 @@ void mf_destroy(mf_ctx* c)
     if (c->h_ds) cudaFreeHost(c->h_ds);
     if (c->partials) cudaFree(c->partials);
     if (c->h_partials) cudaFreeHost(c->h_partials);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     if (c->own_stream) cudaStreamDestroy(c->own_stream);
     for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
     delete c;
@@ -448,6 +459,7 @@ const char* mf_last_error(mf_ctx* c) { return c ? c->err.c_str() : g_create_err.
 int mf_set_stream(mf_ctx* c, void* cuda_stream)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     MF_CUDA(c, cudaStreamSynchronize(c->stream));
     c->stream = cuda_stream ? (cudaStream_t)cuda_stream : c->own_stream;
     return MF_OK;
@@ -469,6 +481,7 @@ int mf_launch_count(mf_ctx* c, long long* launches)
 int mf_profile(mf_ctx* c, int on)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     c->prof_on = on ? 1 : 0;
     return MF_OK;
 }
@@ -595,33 +608,87 @@ int mf_get_state_prim(mf_ctx* c, double* e, double* vx, double* vy, double* vz, 
     return fetch_step_state(c);
 }
 
+// ---- stepping.  One step = (CFL reduction if the accumulator is stale) + per-step scalars + the RK stages; nothing in it needs the host.
+// mode 0: dt = value*dx/S_max (value = cfl); mode 1: dt = value.
+static int enqueue_step(mf_ctx* c, int mode, double value)
+{
+    if (mode == 0 && !c->smax_valid) {                            // otherwise the previous step's last combine already reduced U^n
+        int ps = prof_begin(c, 0);
+        c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->nst), c->ds, c->num_sms, c->stream);   // a2, from U^n
+        prof_end(c, ps);
+    }
+    c->launches += launch_begin_step(c->ds, c->nev, mode, value, c->g.dx, c->alpha, c->stream);
+    return run_step(c);
+}
+
+// Launch-bound grids (config 1: 400 cells, 8 launches of a few microseconds of work each): after one eager step - which allocates the
+// scratch and brings the S_max accumulator into its steady state - a whole period of the register rotation (3 steps, 2 in low-storage
+// mode) is captured into a CUDA graph once and replayed.  Every per-step scalar lives in device memory (StepState), so the replayed
+// launches are exactly the eager ones; what IS baked into the graph (cfl or dt, the option set, the stream, the starting register) is its key.
+static int run_steps(mf_ctx* c, int n, int mode, double value)
+{
+    int done = 0, rc;
+    const int period = c->nreg;                                   // cur returns to its value after this many steps (RK2 and RK3 alike)
+    if (c->graph_on && !c->prof_on && n >= 1 + 2 * period) {
+        if ((rc = enqueue_step(c, mode, value)) != MF_OK) return rc;
+        if ((rc = check_launch(c)) != MF_OK) return rc;
+        done = 1;
+        const bool hit = c->graph_exec && c->graph_epoch == c->epoch && c->graph_cur == c->cur && c->graph_mode == mode &&
+                         c->graph_value == value && c->graph_steps == period;
+        if (!hit) {
+            if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+            const int cur0 = c->cur, smax0 = c->smax_valid;
+            const long long l0 = c->launches;
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                rc = MF_OK;
+                for (int s = 0; s < period && rc == MF_OK; ++s) rc = enqueue_step(c, mode, value);
+                const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+                c->graph_launches = c->launches - l0;
+                c->launches = l0;                                  // nothing ran yet: the capture only recorded
+                c->cur = cur0; c->smax_valid = smax0;
+                if (rc != MF_OK || e != cudaSuccess || !graph || cudaGraphInstantiate(&c->graph_exec, graph, 0) != cudaSuccess) {
+                    cudaGetLastError();
+                    c->graph_exec = nullptr;                       // fall back to eager launches below
+                }
+                if (graph) cudaGraphDestroy(graph);
+            } else cudaGetLastError();
+            if (c->graph_exec) {
+                c->graph_epoch = c->epoch; c->graph_cur = c->cur; c->graph_mode = mode; c->graph_value = value; c->graph_steps = period;
+            }
+        }
+        if (c->graph_exec) {
+            while (n - done >= period) {
+                MF_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
+                c->launches += c->graph_launches;
+                done += period;                                    // cur and smax_valid are back where they were
+            }
+        }
+    }
+    for (; done < n; ++done)
+        if ((rc = enqueue_step(c, mode, value)) != MF_OK) return rc;
+    return check_launch(c);
+}
+
 int mf_step(mf_ctx* c, int n, double cfl)
 {
     if (!c) return MF_EINVAL;
     if (n < 0 || !(cfl > 0.0)) return fail(c, MF_EINVAL, "bad n or cfl");
-    for (int s = 0; s < n; ++s) {
-        if (!c->smax_valid) {                                      // otherwise the previous step's last combine already reduced U^n
-            int ps = prof_begin(c, 0);
-            c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->nst), c->ds, c->num_sms, c->stream);   // a2, from U^n
-            prof_end(c, ps);
-        }
-        c->launches += launch_begin_step(c->ds, c->nev, 0, cfl, c->g.dx, c->alpha, c->stream);
-        int rc = run_step(c);
-        if (rc != MF_OK) return rc;
-    }
-    return check_launch(c);
+    return run_steps(c, n, 0, cfl);
 }
 
 int mf_step_dt(mf_ctx* c, int n, double dt)
 {
     if (!c) return MF_EINVAL;
     if (n < 0 || !(dt > 0.0)) return fail(c, MF_EINVAL, "bad n or dt");
-    for (int s = 0; s < n; ++s) {
-        c->launches += launch_begin_step(c->ds, c->nev, 1, dt, c->g.dx, c->alpha, c->stream);
-        int rc = run_step(c);
-        if (rc != MF_OK) return rc;
-    }
-    return check_launch(c);
+    return run_steps(c, n, 1, dt);
+}
+
+int mf_set_graph(mf_ctx* c, int on)
+{
+    if (!c) return MF_EINVAL;
+    c->graph_on = on ? 1 : 0;
+    return MF_OK;
 }
 
 int mf_eval_L(mf_ctx* c, double dt, double* L_E, double* L_Mx, double* L_My, double* L_Mz, double* L_R)
@@ -714,24 +781,28 @@ int mf_max_signal_speed(mf_ctx* c, double* smax)
 int mf_set_rk(mf_ctx* c, int order)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     if (order != 2 && order != 3) return fail(c, MF_EINVAL, "rk order must be 2 or 3");
     c->rk = order; return MF_OK;
 }
 int mf_set_boundary(mf_ctx* c, int bc)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     if (bc != MF_BC_OUTFLOW && bc != MF_BC_PERIODIC) return fail(c, MF_EINVAL, "unknown boundary condition");
     c->g.periodic = bc == MF_BC_PERIODIC; return MF_OK;
 }
 int mf_set_cs2(mf_ctx* c, double cs2)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     if (!(cs2 > 0.0) || !(cs2 < 1.0)) return fail(c, MF_EINVAL, "cs2 must be in (0,1)");
     set_eos(c->q, cs2); return MF_OK;
 }
 int mf_set_eos_table(mf_ctx* c, int ne, int nn, double ln_e0, double dln_e, double n0, double dn, const double* ln_p)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     if (c->eos != MF_EOS_TABLE) return fail(c, MF_EINVAL, "context was not created with MF_EOS_TABLE");
     if (ne < 2 || nn < 1 || !(dln_e > 0.0) || (nn > 1 && !(dn > 0.0)) || !ln_p) return fail(c, MF_EINVAL, "bad table");
     MF_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -754,6 +825,7 @@ int mf_set_eos_table(mf_ctx* c, int ne, int nn, double ln_e0, double dln_e, doub
 int mf_set_predictor(mf_ctx* c, int on)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     const int keep = c->predictor;
     c->predictor = on ? 1 : 0;
     if (resolve_path(c) != MF_OK) { c->predictor = keep; resolve_path(c); return fail(c, MF_EINVAL, "the selected path does not support this predictor setting: select another path first"); }
@@ -762,12 +834,14 @@ int mf_set_predictor(mf_ctx* c, int on)
 int mf_set_alpha(mf_ctx* c, double alpha)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     if (!(alpha > 0.0)) return fail(c, MF_EINVAL, "alpha must be > 0");
     c->alpha = alpha; return MF_OK;
 }
 int mf_set_jet_source(mf_ctx* c, double dEdx, double sigma, double x0, double y0, double z0)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     if (dEdx != 0.0 && !(sigma > 0.0)) return fail(c, MF_EINVAL, "sigma must be > 0");
     const double PI = 3.14159265358979323846;
     double s2 = sigma > 0.0 ? sigma * sigma : 1.0;
@@ -781,6 +855,7 @@ int mf_set_jet_source(mf_ctx* c, double dEdx, double sigma, double x0, double y0
 int mf_set_path(mf_ctx* c, int path)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     if (path < MF_PATH_AUTO || path > MF_PATH_SWEEP) return fail(c, MF_EINVAL, "unknown path");
     int keep = c->path_req;
     c->path_req = path;
@@ -790,6 +865,7 @@ int mf_set_path(mf_ctx* c, int path)
 int mf_set_low_storage(mf_ctx* c, int on)
 {
     if (!c) return MF_EINVAL;
+    c->epoch++;
     on = on ? 1 : 0;
     if (on == (c->nreg == 2)) return MF_OK;
     MF_CUDA(c, cudaStreamSynchronize(c->stream));

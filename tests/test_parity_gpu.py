@@ -318,3 +318,36 @@ def test_low_storage_path_rules():
     h = MustaForce(16, 16, 16, dx=0.1, path="fused")
     with pytest.raises(MustaForceError):
         h.set_low_storage(True)
+
+
+# ------------------------------------------------------------------ CUDA-graph replay of whole steps
+@pytest.mark.parametrize("shape,kw", [((1, 1, 400), dict(limiter="minmod", k_stages=2, rk=2)),
+                                      ((12, 14, 16), dict(limiter="superbee", k_stages=3, rk=3, bc="periodic")),
+                                      ((12, 14, 16), dict(limiter="mc", k_stages=2, rk=2, predictor=False)),
+                                      ((12, 14, 16), dict(limiter="mc", k_stages=2, rk=3, path="fused"))])
+def test_graph_replay_is_bit_identical_to_eager_launches(shape, kw):
+    """mf_step replays captured steps for n >= 7: same launches, same arguments, so the same bits - across changing n, cfl, fixed-dt steps,
+    option changes (which must invalidate the captured graph) and low-storage mode."""
+    nz, ny, nx = shape
+    st = w.shock_tube_1d() if shape == (1, 1, 400) else w.lumpy_event(shape=shape, dx=0.3, n_gauss=5, radius=1.5, half_z=1.0, background=0.5)
+    out, launches = {}, {}
+    for graph in (True, False):
+        g = MustaForce(nx, ny, nz, dx=st["dx"], **kw)
+        g.set_graph(graph)
+        g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+        g.step(20, 0.3)                                               # 1 eager + 6 replays of 3 + 1 eager
+        g.step(7, 0.3)                                                # same key: the graph is reused
+        g.step(11, 0.25)                                              # another cfl: recaptured
+        g.step_dt(9, 0.004)
+        g._chk(g.lib.mf_set_alpha(g.h, 2.5))                          # option change: the old graph must not be replayed
+        g.step(8, 0.25)
+        if kw.get("path", "auto") == "auto" and kw.get("predictor", True):
+            g.set_low_storage(True)                                   # period 2
+            g.step(9, 0.25)
+        out[graph], launches[graph] = g.get_state(), g.launch_count()
+        assert g.last_status == 0
+        t = g.time()
+        out[graph].append(np.array([t[0], t[1], float(t[2])]))
+    for a, b in zip(out[True], out[False]):
+        assert np.array_equal(a, b)
+    assert launches[True] == launches[False]                          # replayed launches are counted
