@@ -88,10 +88,10 @@ def alg_bytes(rk):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch group at 256^3 (config 3 scheme), one ncu --set full capture per path:
-# staged: k_cell_stage 3.375 GB; k_flux_stage<1>, <2> 2.031 + 2.032 GB; k_xflux_combine 4.721 GB (profiles/r01_ncu_full_staged_256.md)
-# sweep (predictor off): k_sweep_flux<1>, <2> 1.328 + 1.339 GB; k_sweep_xcombine 3.361 GB (profiles/r01_ncu_full_sweep_256.md)
-NCU_TRAFFIC_GB_256 = {("staged", True): {"cell_stage": 3.375, "flux_stage": 4.063, "combine": 4.721},
-                      ("sweep", False): {"flux_stage": 2.667, "combine": 3.361}}
+# staged: k_cell_stage 3.398 GB; k_flux_stage<1>, <2> 2.033 + 2.033 GB; k_xflux_combine 4.719 GB (profiles/r01_ncu_full_staged_256.md)
+# sweep (predictor off): k_sweep_flux<1>, <2> 1.325 + 1.340 GB; k_sweep_xcombine 3.359 GB (profiles/r01_ncu_full_sweep_256.md)
+NCU_TRAFFIC_GB_256 = {("staged", True): {"cell_stage": 3.398, "flux_stage": 4.066, "combine": 4.719},
+                      ("sweep", False): {"flux_stage": 2.665, "combine": 3.359}}
 
 FP64_LANES_PER_SM = 64       # B200 (sm_100): 4 SMSPs x 16 FP64 lanes; mf_probe_fp64 measures it
 
