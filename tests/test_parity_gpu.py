@@ -351,3 +351,18 @@ def test_graph_replay_is_bit_identical_to_eager_launches(shape, kw):
     for a, b in zip(out[True], out[False]):
         assert np.array_equal(a, b)
     assert launches[True] == launches[False]                          # replayed launches are counted
+
+
+# ------------------------------------------------------------------ full-length run of the event configs' scheme (300 steps, guarded states)
+def test_config4_scheme_full_length_300_steps():
+    """BASELINE.json config 4 runs 300 steps; SURVEY probe P5 found that lumpy events on a thin background reach E - |M| -> 0 behind the
+    blast fronts, where only the admissibility guard (A12) keeps the run alive.  Same scheme, reduced box, full length: the CUDA path
+    (fast flux with its integer-pipe admissibility test, guarded fallback) must stay within the bar of the oracle all the way."""
+    st = w.lumpy_event(shape=(28, 32, 36), dx=0.1, n_gauss=8, radius=1.0, half_z=0.6, background=0.02)
+    g, o = parity.make_pair(st)
+    for _ in range(3):
+        g.step(100, st["cfl"])
+        o.step(100, st["cfl"])
+        assert g.sync() == 0 and o.status() == 0
+        parity.assert_parity(g.get_state(), o.get_state(), what="config 4 scheme, %d steps" % g.time()[2])
+    assert g.time()[2] == 300 and g.time()[0] == pytest.approx(o.time()[0], rel=1e-12)
