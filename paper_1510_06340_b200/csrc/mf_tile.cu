@@ -34,7 +34,7 @@ __device__ __forceinline__ double jet_source_t(const Grid& g, const Source& s, i
     double r2 = x * x + y * y + z * z;
     double arg = -r2 * s.inv_two_s2;
 #ifndef MF_STRICT
-    if (arg < -745.0) return 0.0;
+    if (arg < -100.0) return 0.0;            // as in mf_blocks.cuh: below e^-100 of the peak the source is taken as zero
 #endif
     return s.dEdx * s.norm * exp(arg);
 }
