@@ -636,7 +636,10 @@ static int run_steps(mf_ctx* c, int n, int mode, double value)
         const bool hit = c->graph_exec && c->graph_epoch == c->epoch && c->graph_cur == c->cur && c->graph_mode == mode &&
                          c->graph_value == value && c->graph_steps == period;
         if (!hit) {
-            if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+            if (c->graph_exec) {                                   // the old graph may still be running on this stream
+                MF_CUDA(c, cudaStreamSynchronize(c->stream));
+                cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr;
+            }
             const int cur0 = c->cur, smax0 = c->smax_valid;
             const long long l0 = c->launches;
             cudaGraph_t graph = nullptr;
