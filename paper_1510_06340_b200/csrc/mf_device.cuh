@@ -328,7 +328,7 @@ __device__ __forceinline__ double half_slope2(double a, double b)
 
 // ---- fp64 reciprocal and square root for the flux core.
 // The product build uses branch-free Newton sequences seeded by the MUFU approximations (rcp/rsqrt.approx.ftz.f64,
-// ~20 good bits): 3 and 7 FP64-pipe instructions instead of the 9 and 14.5 issue slots that the IEEE-rounded '/' and
+// ~20 good bits): 3 and 6 FP64-pipe instructions instead of the 9 and 14.5 issue slots that the IEEE-rounded '/' and
 // sqrt() cost on B200 (mf_probe_fp64), and no slow-path branch, so independent flux evaluations interleave.
 // Results are within 1 ulp of the correctly rounded value.  The strict build (MF_STRICT)
 // keeps IEEE division and sqrt so that it can be compared with the oracle bit for bit.

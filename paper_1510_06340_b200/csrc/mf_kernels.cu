@@ -395,14 +395,14 @@ int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua,
 }
 
 // =========================================================================== a5 (x) + a7 + a8 (+ a2) in one kernel
-// The x fluxes are the last ones of a stage.  Thread t of a block owns x interface I = 255*block + t (linear over all rows, nx+1 per
-// row), runs MUSTA on it and leaves the flux in shared memory; the cell to the right of the interface then has both of its x fluxes on
-// chip (its own and thread t+1's), reads F_y, F_z of its four other faces, and is finished: divergence, source, RK combine, one store.
-// Blocks overlap by one interface, so 255 of 256 threads finish a cell.  F_x is never written, and the 40 loads of the combine hide
+// The x fluxes are the last ones of a stage.  Thread t of a block of XT threads owns x interface I = (XT-1)*block + t (linear over all rows,
+// nx+1 per row), runs MUSTA on it and leaves the flux in shared memory; the cell to the right of the interface then has both of its x
+// fluxes on chip (its own and thread t+1's), reads F_y, F_z of its four other faces, and is finished: divergence, source, RK combine, one
+// store.  Blocks overlap by one interface, so XT-1 of XT threads finish a cell.  F_x is never written, and the 30 loads of the combine hide
 // under the FP64 work of a compute-bound kernel instead of making a memory-bound pass of their own.
-// 64 registers / 4 blocks per SM: measured on B200, 32 resident warps let the combine's loads of one block overlap the MUSTA of the
-// others (1.37 ms per launch at 256^3 against 1.56 ms at 24 warps; prefetching the operands with cp.async into shared memory at 24
-// warps did not help, 1.53 ms: the kernel is then limited by DRAM bandwidth, not by latency).
+// Measured on B200 (256^3): 128-thread blocks, 5 per SM at 96 registers (the combine's 30 operands are all in flight at once, issued before
+// the barrier); operands prefetched to L2 before MUSTA starts; staging them with cp.async in shared memory instead was 40% slower (the 35 KB
+// per block cost the L1 hits of the x-neighbour loads).  History of this kernel: 1.56 -> 1.37 -> 1.03 -> 0.95 ms per launch.
 // FORM (the RK form of the stage) and CFL (last stage of a step) are compile-time: the stage loop has no form branches, and the
 // signal-speed code with its block reduction exists only in the instantiations that need it.
 template <int EK, int FORM, bool CFL>

@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, i
 
 // =========================================================================== a1 + a3 + a5 (x) + a6 + a7 + a8 (+ a2)
 // The x sweep is the last one of a stage and finishes the cells, like k_xflux_combine of the staged path: thread t of a block owns
-// x interface I = 255*block + t (linear over all rows, nx+1 per row), leaves its MUSTA flux in shared memory, and the cell to the right
+// x interface I = (XT-1)*block + t (linear over all rows, nx+1 per row), leaves its MUSTA flux in shared memory, and the cell to the right
 // of the interface then has both of its x fluxes on chip, reads F_y, F_z of its four other faces, and is done: one store per cell.
 #ifndef MF_XT
 #define MF_XT 128
