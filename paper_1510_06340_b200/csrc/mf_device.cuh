@@ -299,31 +299,23 @@ __device__ __forceinline__ double slope2(double a, double b)
     return ab > 0.0 ? m : 0.0;
 }
 
-// Half the limited slope, 0.5 * slope2(a, b), for the product build's cell stage.  For minmod, superbee and MC the
-// magnitudes are non-negative doubles, whose order is the order of their bit patterns as unsigned integers: min and max
-// are taken on the integer pipe (fmin/fmax on doubles cost a DSETP, two selects, a NaN fix-up and register moves each),
-// and "same sign" is the xor of the sign bits; a zero difference gives lo = 0 and so a zero slope, as ab > 0 does.  Equal
-// to 0.5 * slope2 except where a*b underflows (|slope| < 1e-150 there).
+// Half the limited slope, 0.5 * slope2(a, b), for the product build.  For minmod, superbee and MC the magnitude comparisons are single
+// DSETPs with |.| operand modifiers and the selects act on the SIGNED operands (lo, hi, a+b all carry the sign of a wherever the result is
+// used), so no fmin/fmax (a DSETP, two selects, a NaN fix-up and register moves each on this target), no copysign: 14 instructions for
+// superbee.  An earlier form took min/max on the integer pipe from the bit patterns (~20 instructions, none on the FP64 pipe); measured on
+// B200 the shorter sequence wins even in the FP64-bound sweep kernels (cell stage 0.73 -> 0.67 ms, sweep path 7.19 -> 6.97 ms per step).
+// Equal to 0.5 * slope2 bit for bit: every operation is exact except a + b, which slope2 forms too; "same sign" is a*b > 0 (A6, A16).
 template <int LIM>
 __device__ __forceinline__ double half_slope2(double a, double b)
 {
     if (LIM != LIM_MINMOD && LIM != LIM_SUPERBEE && LIM != LIM_MC) return 0.5 * slope2<LIM>(a, b);
-    const unsigned long long ABS = 0x7fffffffffffffffull;
-    const unsigned long long ia = (unsigned long long)__double_as_longlong(a) & ABS;
-    const unsigned long long ib = (unsigned long long)__double_as_longlong(b) & ABS;
-    const bool a_less = ia < ib;
-    const unsigned long long lo = a_less ? ia : ib, hi = a_less ? ib : ia;
-    unsigned long long h;
-    if (LIM == LIM_MINMOD) h = (unsigned long long)__double_as_longlong(0.5 * __longlong_as_double((long long)lo));
-    else {
-        const double other = LIM == LIM_SUPERBEE ? 0.5 * __longlong_as_double((long long)hi)                                       // min(hi, 2 lo)/2
-                                                 : 0.25 * (__longlong_as_double((long long)hi) + __longlong_as_double((long long)lo));  // min(2 lo, |a+b|/2)/2
-        const unsigned long long io = (unsigned long long)__double_as_longlong(other);
-        h = io < lo ? io : lo;
-    }
-    const int sa = __double2hiint(a), sb = __double2hiint(b);
-    const double r = __hiloint2double((int)(h >> 32) | (sa & (int)0x80000000), (int)(unsigned int)h);
-    return (sa ^ sb) >= 0 ? r : 0.0;
+    const bool a_less = fabs(a) < fabs(b);
+    const double lo = a_less ? a : b, hi = a_less ? b : a;
+    double r;
+    if (LIM == LIM_MINMOD) r = 0.5 * lo;
+    else if (LIM == LIM_SUPERBEE) { const double lo2 = lo + lo; r = 0.5 * (fabs(hi) < fabs(lo2) ? hi : lo2); }      // min(hi, 2 lo)/2
+    else { const double q = 0.25 * (a + b); r = fabs(q) < fabs(lo) ? q : lo; }                                     // min(2 lo, |a+b|/2)/2
+    return a * b > 0.0 ? r : 0.0;
 }
 
 // ---- fp64 reciprocal and square root for the flux core.
