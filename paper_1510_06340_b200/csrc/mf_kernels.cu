@@ -401,8 +401,8 @@ int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua,
 // store.  Blocks overlap by one interface, so XT-1 of XT threads finish a cell.  F_x is never written, and the 30 loads of the combine hide
 // under the FP64 work of a compute-bound kernel instead of making a memory-bound pass of their own.
 // Measured on B200 (256^3): 128-thread blocks, 5 per SM at 96 registers (the combine's 30 operands are all in flight at once, issued before
-// the barrier); operands prefetched to L2 before MUSTA starts; staging them with cp.async in shared memory instead was 40% slower (the 35 KB
-// per block cost the L1 hits of the x-neighbour loads).  History of this kernel: 1.56 -> 1.37 -> 1.03 -> 0.95 ms per launch.
+// the barrier; an extra L2 prefetch of them before MUSTA stopped paying once they were); staging them with cp.async in shared memory
+// instead was 40% slower (the 35 KB per block cost the L1 hits of the x-neighbour loads).  History of this kernel: 1.56 -> 1.37 -> 1.03 -> 0.95 ms per launch.
 // FORM (the RK form of the stage) and CFL (last stage of a step) are compile-time: the stage loop has no form branches, and the
 // signal-speed code with its block reduction exists only in the instantiations that need it.
 template <int EK, int FORM, bool CFL>
@@ -431,16 +431,6 @@ __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q,
 #pragma unroll
         for (int v = 0; v < 5; ++v) { A[v] = fc.f[0][1][v][p] + fc.f[0][0][v][p]; B[v] = fc.f[0][1][v][p + 1] - fc.f[0][0][v][p + 1]; }
 #endif
-        if (t < XT - 1 && f < g.n[0]) {                                    // pull the combine's operands towards L2 while MUSTA runs
-            const unsigned int pc = p + 1, o = eo + f + (unsigned int)j * (unsigned int)g.ns[1] + (unsigned int)kz * (unsigned int)g.ns[2];
-#pragma unroll
-            for (int v = 0; v < 5; ++v) {
-                if (g.act[1]) prefetch_l2(&fx.f[1][v][pc]);      // the neighbour lines (pc - es) are somebody else's pc: prefetching
-                if (g.act[2]) prefetch_l2(&fx.f[2][v][pc]);      // them too measured slower
-                if (FORM != 3) prefetch_l2(&Ua.q[v][o]);
-                if (FORM == 1 || FORM == 2) prefetch_l2(&Ub.q[v][o]);
-            }
-        }
         musta_flux<0, EK>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
     }
     // The combine's operands.  Every one is loaded before the first store: `out` may alias the inputs as far as the compiler knows (and does

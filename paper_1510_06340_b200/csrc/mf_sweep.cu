@@ -143,15 +143,6 @@ __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int li
 #pragma unroll
             for (int v = 0; v < 5; ++v) { A[v] = A[v] + __ldg(&Dl.q[v][p]); B[v] = B[v] + __ldg(&Dl.q[v][p + 1]); }
         }
-        if (t < XT - 1 && f < g.n[0]) {                                    // pull the combine's operands towards L2 while MUSTA runs
-            const unsigned int pc = p + 1, oc = row + f;
-#pragma unroll
-            for (int v = 0; v < 5; ++v) {
-                if (g.act[1]) prefetch_l2(&fx.f[1][v][pc]);
-                if (g.act[2]) prefetch_l2(&fx.f[2][v][pc]);
-                if (FORM == 1 || FORM == 2) prefetch_l2(&Ua.q[v][oc]);       // FORM 0: U^n is V itself, already on its way
-            }
-        }
         musta_flux<0, 0>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
     }
     // The combine's operands: all loaded before the first store (`out` may alias the inputs as far as the compiler knows: loads written after
