@@ -91,7 +91,7 @@ def alg_bytes(rk):
 # staged: k_cell_stage 3.398 GB; k_flux_stage<1>, <2> 2.033 + 2.033 GB; k_xflux_combine 4.719 GB (profiles/r01_ncu_full_staged_256.md)
 # sweep (predictor off): k_sweep_flux<1>, <2> 1.325 + 1.340 GB; k_sweep_xcombine 3.359 GB (profiles/r01_ncu_full_sweep_256.md)
 NCU_TRAFFIC_GB_256 = {("staged", True): {"cell_stage": 3.398, "flux_stage": 4.066, "combine": 4.719},
-                      ("sweep", False): {"flux_stage": 2.665, "combine": 3.359}}
+                      ("sweep", False): {"flux_stage": 2.664, "combine": 3.359}}
 
 FP64_LANES_PER_SM = 64       # B200 (sm_100): 4 SMSPs x 16 FP64 lanes; mf_probe_fp64 measures it
 
