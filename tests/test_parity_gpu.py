@@ -366,3 +366,70 @@ def test_config4_scheme_full_length_300_steps():
         assert g.sync() == 0 and o.status() == 0
         parity.assert_parity(g.get_state(), o.get_state(), what="config 4 scheme, %d steps" % g.time()[2])
     assert g.time()[2] == 300 and g.time()[0] == pytest.approx(o.time()[0], rel=1e-12)
+
+
+# ------------------------------------------------------------------ the BASELINE.json configs at full size AND full length
+def _run_full(st, steps, batch=None):
+    nz, ny, nx = st["shape"]
+    g = MustaForce(nx, ny, nz, dx=st["dx"], batch=batch, **st["scheme"])
+    if "jet" in st:
+        j = st["jet"]
+        g.set_jet_source(j["dEdx"], j["sigma"], j["x0"], j["y0"], j["z0"])
+    return g
+
+
+def test_config3_full_size_500_steps_conserves():
+    """Config 3 as BASELINE.json states it: 256^3 periodic, superbee, k=3, RK3, 500 steps; total E, M and R conserved to round-off (Q2)."""
+    st = w.gaussian_hot_spot()
+    g = _run_full(st, 500)
+    g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+    t0 = g.totals()
+    g.step(500, st["cfl"])
+    t1 = g.totals()
+    assert g.sync() == 0 and g.time()[2] == 500
+    assert abs(t1[0] - t0[0]) / t0[0] <= 1e-12 and abs(t1[4] - t0[4]) / t0[4] <= 1e-12
+    assert max(abs(t1[q]) for q in (1, 2, 3)) / t0[0] <= 1e-12
+    E = g.get_state()[0]
+    assert np.all(np.isfinite(E)) and E.min() > 0.0
+
+
+def test_config2_full_size_200_steps_runs_clean():
+    """Config 2 as BASELINE.json states it (128^3 diagonal shock, MC, k=2, RK2, 200 steps): admissible to the end, sticky status clear."""
+    st = w.diagonal_shock_3d()
+    g = _run_full(st, 200)
+    g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+    g.step(200, st["cfl"])
+    assert g.sync() == 0
+    U = g.get_state()
+    assert np.all(np.isfinite(U[0])) and np.all(U[0] > np.sqrt(U[1] ** 2 + U[2] ** 2 + U[3] ** 2))
+
+
+def test_config4_batch_full_size_300_steps():
+    """Config 4: eight of the 32 seeded 128^3 events in one batch, the full 300 steps.  Behind the blast fronts E - |M| falls to 1e-4 and
+    in some events a stored cell is transiently superluminal (SURVEY probe P5): the sticky MF_ESTATE flag may then be raised - the oracle
+    raises it at the same step, see the next test - while the guard (A12) keeps every event finite and running on its own clock."""
+    events = [w.lumpy_event(event=ev) for ev in range(8)]
+    g = _run_full(events[0], 300, batch=8)
+    g.set_state(*[np.stack([ev[f] for ev in events]) for f in ("E", "Mx", "My", "Mz", "R")])
+    g.step(300, events[0]["cfl"])
+    assert g.sync() in (0, MF_ESTATE)
+    U = g.get_state()
+    assert all(np.all(np.isfinite(a)) for a in U) and U[0].min() > 0.0
+    assert all(g.time(ev)[2] == 300 for ev in range(8))
+    assert len({g.time(ev)[0] for ev in range(8)}) == 8                # eight different clocks
+
+
+def test_config4_event_full_size_parity_with_status():
+    """One config-4 event (seed 20151006 + 5) at FULL size against the oracle over the 150 steps in which a stored cell becomes superluminal:
+    same state within the bar, same dt sequence, and the sticky status raised by both in the same window."""
+    st = w.lumpy_event(event=5)
+    g, o = parity.make_pair(st)
+    seen = []
+    for s in range(0, 150, 25):
+        g.step(25, st["cfl"])
+        o.step(25, st["cfl"])
+        seen.append((g.sync(), o.status()))
+        assert seen[-1][0] == seen[-1][1]
+    assert seen[0] == (0, 0) and seen[-1] == (MF_ESTATE, MF_ESTATE)
+    parity.assert_parity(g.get_state(), o.get_state(), what="config 4, event 5, 128^3, 150 steps")
+    assert g.time()[0] == pytest.approx(o.time()[0], rel=1e-12)
