@@ -433,3 +433,21 @@ def test_config4_event_full_size_parity_with_status():
     assert seen[0] == (0, 0) and seen[-1] == (MF_ESTATE, MF_ESTATE)
     parity.assert_parity(g.get_state(), o.get_state(), what="config 4, event 5, 128^3, 150 steps")
     assert g.time()[0] == pytest.approx(o.time()[0], rel=1e-12)
+
+
+def test_config5_full_size_400_steps():
+    """Config 5 as BASELINE.json states it: 512^3 lumpy event with the moving jet source, MC, k=3, RK3, the full 400 steps (largest grid:
+    5 GB per state register, 64 GB with the staged scratch).  Finite and positive to the end; while nothing has left the box the source's
+    energy budget holds (Q10): total E and total Mx grow by dE/dx per unit time."""
+    st = w.jet_event()
+    g = _run_full(st, 400)
+    g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+    t0 = g.totals()
+    g.step(40, st["cfl"])                                              # t ~ 0.6 fm: the fronts are still 4 fm from the faces
+    t1, tm = g.totals(), g.time()[0]
+    dEdx = st["jet"]["dEdx"]
+    assert t1[0] - t0[0] == pytest.approx(dEdx * tm, rel=1e-6) and t1[1] - t0[1] == pytest.approx(dEdx * tm, rel=1e-6)
+    g.step(360, st["cfl"])
+    assert g.sync() in (0, MF_ESTATE) and g.time()[2] == 400
+    E = g.get_state()[0]
+    assert np.all(np.isfinite(E)) and E.min() > 0.0
