@@ -451,3 +451,29 @@ def test_config5_full_size_400_steps():
     assert g.sync() in (0, MF_ESTATE) and g.time()[2] == 400
     E = g.get_state()[0]
     assert np.all(np.isfinite(E)) and E.min() > 0.0
+
+
+def test_config2_full_size_parity_100_steps():
+    """BASELINE.json's bar taken literally for config 2: the whole 128^3 grid, 100 steps, every cell against the oracle (OpenMP build, bit-identical
+    to the one-thread oracle)."""
+    st = w.diagonal_shock_3d()
+    g, o = parity.make_pair(st)
+    g.step(100, st["cfl"])
+    o.step(100, st["cfl"])
+    assert g.sync() == 0 and o.status() == 0
+    r = parity.assert_parity(g.get_state(), o.get_state(), what="config 2 at 128^3, 100 steps")
+    assert g.time()[0] == pytest.approx(o.time()[0], rel=1e-12)
+    print("config 2 full size: rel diff E,M,R =", r)
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("MF_LONG_TESTS"), reason="~8 min of oracle time on 16 host threads; set MF_LONG_TESTS=1 (result recorded in BASELINE.md)")
+def test_config3_full_size_parity_100_steps():
+    """BASELINE.json's bar taken literally for the metric's workload: the whole 256^3 grid, 100 steps, every cell against the oracle."""
+    st = w.gaussian_hot_spot()
+    g, o = parity.make_pair(st)
+    g.step(100, st["cfl"])
+    o.step(100, st["cfl"])
+    assert g.sync() == 0 and o.status() == 0
+    r = parity.assert_parity(g.get_state(), o.get_state(), what="config 3 at 256^3, 100 steps")
+    assert g.time()[0] == pytest.approx(o.time()[0], rel=1e-12)
+    print("config 3 full size: rel diff E,M,R =", r)
