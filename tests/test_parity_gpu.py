@@ -467,13 +467,16 @@ def test_config2_full_size_parity_100_steps():
 
 
 @pytest.mark.skipif(not __import__("os").environ.get("MF_LONG_TESTS"), reason="~8 min of oracle time on 16 host threads; set MF_LONG_TESTS=1 (result recorded in BASELINE.md)")
-def test_config3_full_size_parity_100_steps():
-    """BASELINE.json's bar taken literally for the metric's workload: the whole 256^3 grid, 100 steps, every cell against the oracle."""
+@pytest.mark.parametrize("predictor", [True, False])
+def test_config3_full_size_parity_100_steps(predictor):
+    """BASELINE.json's bar taken literally for the metric's workload: the whole 256^3 grid, 100 steps, every cell against the oracle - on the
+    staged path (Hancock predictor on, the default) and on the sweep path (predictor off)."""
     st = w.gaussian_hot_spot()
-    g, o = parity.make_pair(st)
+    g, o = parity.make_pair(st, predictor=predictor)
+    assert g.path() == ("staged" if predictor else "sweep")
     g.step(100, st["cfl"])
     o.step(100, st["cfl"])
     assert g.sync() == 0 and o.status() == 0
     r = parity.assert_parity(g.get_state(), o.get_state(), what="config 3 at 256^3, 100 steps")
     assert g.time()[0] == pytest.approx(o.time()[0], rel=1e-12)
-    print("config 3 full size: rel diff E,M,R =", r)
+    print("config 3 full size, predictor", predictor, ": rel diff E,M,R =", r)
