@@ -491,8 +491,7 @@ __device__ __forceinline__ void musta_flux(const Eos& q, int k, double lam, doub
     }
 #pragma unroll
     for (int c = 0; c < 5; ++c) F[c] = 0.5 * F[c];
-    return;
-    }
+    } else
 #endif
     for (int l = 0;; ++l) {
         double FA[5], FB[5], W[5];

@@ -291,8 +291,8 @@ __global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, 
     const unsigned int p = blockIdx.y * (unsigned int)g.next + (c[0] + g.h[0]) * es[0] + (c[1] + g.h[1]) * es[1] + (c[2] + g.h[2]) * es[2];   // < 2^32 (mf_create)
     ds += blockIdx.y;
     double A[5], B[5], F[5];
-#pragma unroll
 #ifdef MF_STRICT
+#pragma unroll
     for (int v = 0; v < 5; ++v) { A[v] = fc.f[D][1][v][p]; B[v] = fc.f[D][0][v][p + es[D]]; }   // A2 :173
 #else
     {                                                                                             // compact scratch: W and H_D
