@@ -239,6 +239,12 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
                 const long long o = co + (long long)kc * ns2;
                 double S = 0.0;
                 if (src.on) S = jet_source_t(g, src, gx, gy, kc, ds->t + sg.ts * dt);
+                double ua5[5], ub5[5];                                   // loaded before the first store (`out` may alias them for all the compiler knows)
+#pragma unroll
+                for (int v = 0; v < 5; ++v) {
+                    ua5[v] = sg.form == 3 ? 0.0 : Ua.q[v][o];
+                    ub5[v] = (sg.form == 1 || sg.form == 2) ? V.q[v][o] : 0.0;
+                }
 #pragma unroll
                 for (int v = 0; v < 5; ++v) {
                     double acc = s_xy[v][t] + (F[v] - s_Fz[v][t]);
@@ -248,9 +254,7 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
                     double L = -acc * g.inv_dx;
 #endif
                     if (src.on && v < 2) L = L + S;
-                    double ua = sg.form == 3 ? 0.0 : Ua.q[v][o];
-                    double ub = (sg.form == 1 || sg.form == 2) ? V.q[v][o] : 0.0;
-                    out.q[v][o] = rk_form_t(sg, ua, ub, dt, L);
+                    out.q[v][o] = rk_form_t(sg, ua5[v], ub5[v], dt, L);
                 }
             }
 #pragma unroll
