@@ -21,7 +21,11 @@
  * Pins (tests/, -m "not gpu"): exact p=e/3 Riemann solution under refinement (Q1), conservation on a
  * periodic box (Q2), uniform-state fixed point (Q3), axis-permutation symmetry (Q4), Eq.4<->Eq.23 round
  * trip (Q5), limiter identities vs Eq.18-22 (Q6), first-order FORCE closed-form stencil on linear
- * advection (Q7), limiter/k ordering (Q8), numpy transcription on tiny inputs (Q9), source budget (Q10).
+ * advection (Q7), limiter/k ordering (Q8), numpy transcription on tiny inputs (Q9), source budget (Q10),
+ * the MUSTA_k predictor-corrector update Eq.8 against its closed form in k for a linear flux (a geometric
+ * sequence; tests/test_oracle_pieces.py::test_musta_linear_flux_closed_form), the signal speed at rest / at
+ * |v| -> 1 / as a sum of rapidities, and the source's RK stage times as the nodes of the trapezoidal and
+ * Simpson rules on a one-cell grid (error orders dt^3, dt^5 against the exact erf integral).
  * PARITY UNPINNED by the paper (definitions of ours): accuracy effect of running the
  * Hancock half step inside every RK stage (A4), admissibility-guard constants (A12), jet source
  * definition (A14), charge profile (A13).

@@ -210,3 +210,85 @@ def test_musta_flux_mirror_symmetry():
     F = o.musta_flux(0, 0.35, A, B)
     G = o.musta_flux(0, 0.35, B * flip, A * flip)
     assert np.allclose(G, F * np.array([-1, 1, -1, -1, -1.0]), rtol=1e-13, atol=1e-15)
+
+
+# ---------------------------------------------------------------- MUSTA_k on a linear flux: closed form in k (pins Eq.8)
+@pytest.mark.parametrize("alpha", [1.0, 3.0])
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_musta_linear_flux_closed_form(alpha, d):
+    """Eq.8-11 for a LINEAR flux f = c u have a closed form in k, derived here from the paper's equations and
+    not from any code: with s = u_L + u_R, j = u_R - u_L and D = (alpha lam c^2 + 1/(alpha lam))/2,
+        Eq.10:  u_lw = s/2 - (alpha lam/2) c j          Eq.11:  f_lf = c s/2 - j/(2 alpha lam)
+        Eq.9:   F    = c s/2 - D j/2
+        Eq.8:   s'   = s - lam c j,   j' = j (1 - lam D)
+    so j_l = j_0 q^l with q = 1 - lam D (a geometric sequence), s_l = s_0 - (c/D) j_0 (1 - q^l), and
+        F^(k) = c s_0/2 - j_0 (c^2/(2D) (1 - q^k) + (D/2) q^k).
+    The R equation of Eq.3 is exactly this when E and M are equal on both sides: they stay equal through every
+    stage (their fluxes coincide), so v_d = c is one constant and F_R = c R.  A wrong factor, sign or index in Eq.8 changes q."""
+    e0, v = 2.0, np.array([0.4, -0.3, 0.25])
+    c = v[d]
+    lam = 0.3
+    for k in range(0, 6):
+        o = Oracle(8, dx=1.0, k_stages=k, alpha=alpha)
+        UL = o.prim2con([e0, *v, 1.7])
+        UR = o.prim2con([e0, *v, 0.6])
+        assert np.all(UL[:4] == UR[:4])
+        F = o.musta_flux(d, lam, UL, UR)
+        s0, j0 = UL[4] + UR[4], UR[4] - UL[4]
+        D = 0.5 * (alpha * lam * c * c + 1.0 / (alpha * lam))
+        q = 1.0 - lam * D
+        want = 0.5 * c * s0 - j0 * (c * c / (2.0 * D) * (1.0 - q ** k) + 0.5 * D * q ** k)
+        assert F[4] == pytest.approx(want, rel=1e-14, abs=1e-15), (k, F[4], want)
+        assert np.allclose(F[:4], o.flux(d, UL)[:4], rtol=1e-14, atol=1e-15)        # E, M: the physical flux, untouched by the stages
+    # the stages matter: k = 0 and k = 3 differ by far more than the tolerance above (so the test can see Eq.8)
+    assert abs((1.0 - q ** 3) * (c * c / (2.0 * D) - 0.5 * D) * j0) > 1e-3
+
+
+# ---------------------------------------------------------------- signal speed (A10): special cases and the velocity-addition identity
+def test_max_signal_speed_special_cases():
+    """S = (|v| + c_s)/(1 + |v| c_s) is the relativistic sum of |v| and c_s: equal to c_s for matter at rest, increasing in |v|,
+    below 1 and tending to 1 as |v| -> 1, and tanh(artanh|v| + artanh c_s) (rapidities add)."""
+    for cs2 in (1.0 / 3.0, 0.2):
+        cs = math.sqrt(cs2)
+        o = Oracle(4, dx=1.0, cs2=cs2)
+        one = np.ones(4)
+        o.set_state_prim(2.0 * one, 0 * one, 0 * one, 0 * one, one)
+        assert o.max_signal_speed()[0] == pytest.approx(cs, rel=1e-15)
+        last = cs
+        for vmag in (0.1, 0.5, 0.9, 0.99, 0.9999, 0.999999):
+            vx, vy, vz = vmag * 0.6, -vmag * 0.48, vmag * 0.64                         # |v| = vmag in a general direction
+            o.set_state_prim(np.array([1.0, 2.0, 3.0, 0.5]), vx * one, vy * one, vz * one, one)
+            s = o.max_signal_speed()[0]
+            assert s == pytest.approx(math.tanh(math.atanh(vmag) + math.atanh(cs)), rel=1e-9 / (1 - vmag))
+            assert last < s < 1.0
+            last = s
+        assert 1.0 - last < 1e-6
+
+
+# ---------------------------------------------------------------- RK stage times of the source (A14): quadrature order on a single cell
+@pytest.mark.parametrize("rk,order", [(2, 3), (3, 5)])
+def test_source_stage_times_are_the_quadrature_nodes(rk, order):
+    """On a grid of ONE cell nothing flows, so a step integrates dE/dt = S(t) alone and Eq.6 / Eq.7 become
+    quadrature rules: RK2 with the source taken at t, t+dt is the trapezoidal rule, RK3 with t, t+dt, t+dt/2 is Simpson's rule.
+    Against the exact integral (an error function) the one-step error must then fall as dt^3 and dt^5; any other stage time
+    leaves an O(dt^2) error, and any other weight an O(dt) one."""
+    dEdx, sig, x0 = 5.0, 0.5, -1.5                 # the pulse's leading flank: its derivatives keep their sign over [0, dt]
+    amp = dEdx * (2 * math.pi * sig * sig) ** -1.5
+
+    def exact(dt):                                  # integral of amp exp(-(x0+t)^2/(2 sig^2)) over [0, dt]; the cell centre sits at x = 0
+        r = sig * math.sqrt(2.0)
+        return amp * sig * math.sqrt(math.pi / 2) * (math.erf((x0 + dt) / r) - math.erf(x0 / r))
+
+    errs = []
+    for dt in (0.2, 0.1, 0.05):
+        o = Oracle(1, 1, 1, dx=0.25, rk=rk)
+        o.set_state([2.0], [0.0], [0.0], [0.0], [1.0])
+        o.set_jet_source(dEdx, sig, x0, 0.0, 0.0)
+        o.step_dt(1, dt)
+        U = [u.ravel()[0] for u in o.get_state()]
+        assert U[1] == pytest.approx(U[0] - 2.0, rel=1e-14)          # S_Mx = S_E
+        assert U[2] == 0.0 and U[3] == 0.0 and U[4] == 1.0
+        errs.append(abs((U[0] - 2.0) - exact(dt)))
+        assert errs[-1] < 0.15 * exact(dt)
+    for a, b in zip(errs, errs[1:]):
+        assert 2 ** order * 0.7 < a / b < 2 ** order * 1.4, (errs, order)
