@@ -71,7 +71,7 @@ void    mf_destroy(mf_ctx*);
  * dt = cfl*dx/S_max(event) on the device, so an event of the batch evolves exactly as it would alone in an mf_create context.
  * Every state array of the calls below then holds nevents*nx*ny*nz doubles, event-major: idx = cell + nx*ny*nz*event.  Scheme options
  * (limiter, RK, boundary, EOS, source, ...) are shared by the batch.  1 <= nevents <= 65535, nevents*(cells with boundary layer) < 2^32;
- * runs on the staged path.  mf_create(...) is mf_create_batch(1, ...). */
+ * runs on the staged path, or on the sweep path when the Hancock predictor is off (MF_PATH_AUTO).  mf_create(...) is mf_create_batch(1, ...). */
 mf_ctx* mf_create_batch(int nevents, int nx, int ny, int nz, double dx, int eos, int limiter, int k_stages);
 int mf_batch_size(mf_ctx*);                 /* nevents (1 for mf_create) */
 
@@ -128,6 +128,9 @@ int mf_set_low_storage(mf_ctx*, int on);
  * ones (every per-step scalar lives in device memory), so results are bit-identical; it removes the per-launch host cost that dominates
  * small grids.  On by default; off while mf_profile is recording.  mf_set_graph(ctx, 0) forces eager launches. */
 int mf_set_graph(mf_ctx*, int on);
+/* Diagnostic: how many times this context captured a graph and how many times it launched one (either pointer may be NULL).  Repeated
+ * mf_step(n) calls with the same cfl (or dt) and options reuse one capture whatever n is. */
+int mf_graph_stats(mf_ctx*, long long* captures, long long* replays);
 /* Device memory currently held by the context (state registers, scratch allocated so far, tables), in bytes. */
 int mf_memory_bytes(mf_ctx*, long long* bytes);
 /* Run on a caller-owned CUDA stream (a cudaStream_t passed as void*), e.g. PyTorch's current stream, so the
@@ -150,10 +153,12 @@ enum { MF_NCLASS = 8 };
 int mf_profile(mf_ctx*, int on);
 int mf_profile_read(mf_ctx*, double ms[MF_NCLASS], long long launches[MF_NCLASS]);
 
-/* Measured FP64-pipe issue rates of the current device: runs register-only loops of dependent-chain-free
- * DFMA, DADD, DMUL, reciprocal and square root and writes instructions (or results) per second:
- * out = { dfma/s, dadd/s, dmul/s, rcp results/s, sqrt results/s, SM clock estimate in Hz, SM count }. */
-int mf_probe_fp64(double out[7]);
+/* DIAGNOSTIC, not part of the hot path (bench.py calls it for the roofline denominators; MEASURED_PEAKS.json has no FP64 entry).
+ * Measured FP64-pipe issue rates of the current device: runs register-only loops of dependent-chain-free DFMA, DADD, DMUL,
+ * reciprocal and square root and writes instructions (or results) per second:
+ * out = { dfma/s with two register operands (x*a+a), dadd/s, dmul/s, rcp results/s, sqrt results/s, SM clock estimate in Hz, SM count,
+ *         dfma/s with three distinct register operands (x = y*z + x; the register file delivers them in 3 cycles instead of 2) }. */
+int mf_probe_fp64(double out[8]);
 /* Library build info: "mustaforce <version> sm_100a [strict]" */
 const char* mf_version(void);
 

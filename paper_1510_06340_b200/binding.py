@@ -52,6 +52,7 @@ SIGNATURES = {
     "mf_get_path": (C.c_int, [_vp, C.POINTER(C.c_int)]),
     "mf_set_low_storage": (C.c_int, [_vp, C.c_int]),
     "mf_set_graph": (C.c_int, [_vp, C.c_int]),
+    "mf_graph_stats": (C.c_int, [_vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]),
     "mf_memory_bytes": (C.c_int, [_vp, C.POINTER(C.c_longlong)]),
     "mf_set_stream": (C.c_int, [_vp, _vp]),
     "mf_sync": (C.c_int, [_vp]),
@@ -99,12 +100,12 @@ def _f64(a, n):
 
 
 def probe_fp64(strict=False):
-    out = np.zeros(7)
+    out = np.zeros(8)
     rc = load(strict).mf_probe_fp64(_p(out))
     if rc != MF_OK:
         raise MustaForceError(rc, "mf_probe_fp64 failed (no GPU?)")
     return dict(dfma_per_s=out[0], dadd_per_s=out[1], dmul_per_s=out[2], rcp_per_s=out[3], sqrt_per_s=out[4],
-                sm_clock_hz=out[5], sms=int(out[6]))
+                sm_clock_hz=out[5], sms=int(out[6]), dfma3_per_s=out[7])
 
 
 def version(strict=False):
@@ -240,6 +241,11 @@ class MustaForce:
 
     def set_graph(self, on):
         self._chk(self.lib.mf_set_graph(self.h, 1 if on else 0))
+
+    def graph_stats(self):
+        cap, rep = C.c_longlong(), C.c_longlong()
+        self._chk(self.lib.mf_graph_stats(self.h, C.byref(cap), C.byref(rep)))
+        return cap.value, rep.value
 
     def memory_bytes(self):
         b = C.c_longlong()

@@ -35,34 +35,59 @@ def _deps():
         [os.path.join(INCLUDE, "mustaforce.h"), os.path.abspath(__file__)]
 
 
-def _stale(out):
-    if not os.path.exists(out):
+def _newer(target, deps):
+    if not os.path.exists(target):
         return True
-    t = os.path.getmtime(out)
-    return any(os.path.getmtime(p) > t for p in _deps())
+    t = os.path.getmtime(target)
+    return any(os.path.getmtime(p) > t for p in deps)
 
 
-def _compile(out, extra, verbose):
-    cmd = [NVCC] + ARCH + COMMON + extra + sources() + ["-o", out + ".tmp"]
+def _run(cmd, log, verbose):
     if verbose:
         print(" ".join(cmd), file=sys.stderr)
     res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
-    log = out.replace(".so", ".build.log")
-    with open(log, "w") as f:
+    with open(log, "a") as f:
         f.write(" ".join(cmd) + "\n" + res.stdout)
     if res.returncode != 0:
         sys.stderr.write(res.stdout)
-        raise RuntimeError("nvcc failed for %s (log: %s)" % (out, log))
+        raise RuntimeError("nvcc failed: %s (log: %s)" % (cmd[-1], log))
     if verbose:
         sys.stderr.write(res.stdout)
-    os.replace(out + ".tmp", out)
+
+
+def _compile(out, extra, verbose, force):
+    """One object per .cu (compiled in parallel, kept under build/ next to the library, rebuilt when a source or header is newer),
+    then one link."""
+    tag = os.path.basename(out).replace(".so", "")
+    objdir = os.path.join(HERE, "build", tag)
+    os.makedirs(objdir, exist_ok=True)
+    log = out.replace(".so", ".build.log")
+    open(log, "w").close()
+    headers = [p for p in _deps() if not p.endswith(".cu")]
+    flags = [f for f in COMMON if f != "-shared"]
+    jobs, objs = [], []
+    for src in sources():
+        obj = os.path.join(objdir, os.path.basename(src).replace(".cu", ".o"))
+        objs.append(obj)
+        if force or _newer(obj, [src] + headers):
+            jobs.append([NVCC] + ARCH + flags + extra + ["-c", src, "-o", obj])
+    if jobs:
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
+            list(ex.map(lambda cmd: _run(cmd, log, verbose), jobs))
+    if jobs or force or _newer(out, objs):
+        _run([NVCC] + ARCH + ["-shared", "-Xcompiler", "-fPIC"] + objs + ["-o", out + ".tmp"], log, verbose)
+        os.replace(out + ".tmp", out)
 
 
 def build(force=False, verbose=False, strict=True):
-    if force or _stale(LIB):
-        _compile(LIB, [], verbose)
-    if strict and (force or _stale(LIB_STRICT)):
-        _compile(LIB_STRICT, ["--fmad=false", "-DMF_STRICT"], verbose)
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=2) as ex:                    # the two variants side by side
+        futs = [ex.submit(_compile, LIB, [], verbose, force)]
+        if strict:
+            futs.append(ex.submit(_compile, LIB_STRICT, ["--fmad=false", "-DMF_STRICT"], verbose, force))
+        for f in futs:
+            f.result()
     return LIB, LIB_STRICT
 
 

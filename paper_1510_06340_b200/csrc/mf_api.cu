@@ -55,6 +55,7 @@ struct mf_ctx {
     int graph_cur, graph_mode, graph_steps;
     double graph_value;
     long long graph_launches;
+    long long graph_captures, graph_replays;   // diagnostics (mf_graph_stats)
     int prof_on;
     std::vector<cudaEvent_t> prof_ev;     // pairs: [2i] start, [2i+1] stop
     std::vector<int> prof_cls;            // class of pair i
@@ -410,7 +411,7 @@ mf_ctx* mf_create_batch(int nevents, int nx, int ny, int nz, double dx, int eos,
     c->path_req = MF_PATH_AUTO; c->cur = 0; c->nreg = 3; c->launches = 0;
     c->prof_on = 0; c->prof_used = 0; c->smax_valid = 0;
     c->graph_on = 1; c->epoch = 0; c->graph_exec = nullptr; c->graph_epoch = 0; c->graph_cur = -1; c->graph_mode = -1; c->graph_steps = 0;
-    c->graph_value = 0.0; c->graph_launches = 0;
+    c->graph_value = 0.0; c->graph_launches = 0; c->graph_captures = 0; c->graph_replays = 0;
     resolve_path(c);
     c->nblocks_tot = c->num_sms * 4;
 
@@ -501,7 +502,7 @@ int mf_profile_read(mf_ctx* c, double ms[MF_NCLASS], long long launches[MF_NCLAS
     return MF_OK;
 }
 
-int mf_probe_fp64(double out[7])
+int mf_probe_fp64(double out[8])
 {
     if (!out) return MF_EINVAL;
     int ndev = 0;
@@ -633,9 +634,17 @@ static int run_steps(mf_ctx* c, int n, int mode, double value)
         if ((rc = enqueue_step(c, mode, value)) != MF_OK) return rc;
         if ((rc = check_launch(c)) != MF_OK) return rc;
         done = 1;
-        const bool hit = c->graph_exec && c->graph_epoch == c->epoch && c->graph_cur == c->cur && c->graph_mode == mode &&
-                         c->graph_value == value && c->graph_steps == period;
+        const bool same_key = c->graph_exec && c->graph_epoch == c->epoch && c->graph_mode == mode && c->graph_value == value &&
+                              c->graph_steps == period;
+        // The captured period starts from one particular state register.  A call whose step count is not a multiple of the period leaves
+        // U^n in another one: walk there with at most period - 1 eager steps instead of throwing the graph away.
+        while (same_key && c->graph_cur != c->cur && n - done > period) {
+            if ((rc = enqueue_step(c, mode, value)) != MF_OK) return rc;
+            ++done;
+        }
+        const bool hit = same_key && c->graph_cur == c->cur;
         if (!hit) {
+            c->graph_captures++;
             if (c->graph_exec) {                                   // the old graph may still be running on this stream
                 MF_CUDA(c, cudaStreamSynchronize(c->stream));
                 cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr;
@@ -663,6 +672,7 @@ static int run_steps(mf_ctx* c, int n, int mode, double value)
         if (c->graph_exec) {
             while (n - done >= period) {
                 MF_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
+                c->graph_replays++;
                 c->launches += c->graph_launches;
                 done += period;                                    // cur and smax_valid are back where they were
             }
@@ -691,6 +701,14 @@ int mf_set_graph(mf_ctx* c, int on)
 {
     if (!c) return MF_EINVAL;
     c->graph_on = on ? 1 : 0;
+    return MF_OK;
+}
+
+int mf_graph_stats(mf_ctx* c, long long* captures, long long* replays)
+{
+    if (!c) return MF_EINVAL;
+    if (captures) *captures = c->graph_captures;
+    if (replays) *replays = c->graph_replays;
     return MF_OK;
 }
 
@@ -777,7 +795,7 @@ int mf_max_signal_speed(mf_ctx* c, double* smax)
     memcpy(smax, &bits, sizeof(double));
     // leave the accumulators empty for the next reduction
     c->smax_valid = 0;
-    for (int ev = 0; ev < c->nev; ++ev) cudaMemsetAsync(&c->ds[ev].smax_bits, 0, sizeof(unsigned long long), c->stream);
+    cudaMemset2DAsync(&c->ds[0].smax_bits, sizeof(StepState), 0, sizeof(unsigned long long), (size_t)c->nev, c->stream);   // one strided memset for all events
     return rc;
 }
 
@@ -800,7 +818,9 @@ int mf_set_cs2(mf_ctx* c, double cs2)
     if (!c) return MF_EINVAL;
     c->epoch++;
     if (!(cs2 > 0.0) || !(cs2 < 1.0)) return fail(c, MF_EINVAL, "cs2 must be in (0,1)");
-    set_eos(c->q, cs2); return MF_OK;
+    set_eos(c->q, cs2);
+    c->smax_valid = 0;                                             // the accumulator holds S_max for the old sound speed
+    return MF_OK;
 }
 int mf_set_eos_table(mf_ctx* c, int ne, int nn, double ln_e0, double dln_e, double n0, double dn, const double* ln_p)
 {

@@ -54,4 +54,12 @@ __device__ __forceinline__ double jet_source(const Grid& g, const Source& s, int
     return s.dEdx * s.norm * exp(arg);
 }
 
+__device__ __forceinline__ double rk_form(const Stage& sg, double ua, double ub, double dt, double L)
+{
+    if (sg.form == 0) return ua + dt * L;                          // U + dt L            (Eq.6/7 first line)
+    if (sg.form == 1) return 0.5 * (ua + ub + dt * L);             // Eq.6 second line :105
+    if (sg.form == 2) return sg.ca * ua + sg.cb * ub + (sg.cdt * dt) * L;   // Eq.7 lines 2, 3 :112-114
+    return L;                                                      // form 3: L itself (mf_eval_L)
+}
+
 } // namespace mf

@@ -415,7 +415,9 @@ __device__ __forceinline__ bool flux_fast(const Eos& q, const double (&U)[5], do
     const double EE = E * E;
     // admissible and not vacuum, decided on the integer pipe: E > ~1e-12 (high word) and |M|^2 < E^2 by at least one unit of the
     // high word (2^-21 relative, so |M| <= V_CAP E holds with room to spare); anything closer takes the guarded general path
-    const bool ok = (__double2hiint(E) > 0x3D719799) && (__double2hiint(M2) < __double2hiint(EE));
+    // The words are compared as UNSIGNED numbers with one unit of room (the high word of |M|^2 at least TWO below that of E^2): a NaN of
+    // either sign in M (CUDA's canonical NaN has the sign bit set) is larger than every finite E^2 and fails the test.
+    const bool ok = (__double2hiint(E) > 0x3D719799) && ((unsigned int)__double2hiint(M2) + 1u < (unsigned int)__double2hiint(EE));
     const double Qh = sqrt_pos(fma(-q.cs2, M2, q.qc1sq * EE));
     double y;
     {
@@ -525,7 +527,9 @@ __device__ __forceinline__ double signal_speed(const Eos& q, double E, double Mx
         // root and reciprocal, one more Newton root, one more Newton reciprocal.  Everything else takes the general path below.
         const double M2 = fma(Mz, Mz, fma(My, My, Mx * Mx)), EE = E * E;
         const int hEE = __double2hiint(EE);
-        if (__double2hiint(E) > 0x3D719799 && hEE < 0x7ff00000 && __double2hiint(M2) < hEE && (__double2hiint(R) & 0x7fffffff) < 0x7ff00000) {
+        // (unsigned compare with a unit of room: a NaN of either sign in M compares above every finite E^2 and takes the general path)
+        if (__double2hiint(E) > 0x3D719799 && hEE < 0x7ff00000 && (unsigned int)__double2hiint(M2) + 1u < (unsigned int)hEE &&
+            (__double2hiint(R) & 0x7fffffff) < 0x7ff00000) {
             const double Qh = sqrt_pos(fma(-q.cs2, M2, q.qc1sq * EE));
             const double y = rcp_pos(fma(q.hc1, E, Qh));
             const double av2 = M2 * (y * y);

@@ -325,14 +325,6 @@ int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, F
 }
 
 // =========================================================================== a7 + a8: divergence, source, RK combine
-__device__ __forceinline__ double rk_form(const Stage& sg, double ua, double ub, double dt, double L)
-{
-    if (sg.form == 0) return ua + dt * L;                          // U + dt L            (Eq.6/7 first line)
-    if (sg.form == 1) return 0.5 * (ua + ub + dt * L);             // Eq.6 second line :105
-    if (sg.form == 2) return sg.ca * ua + sg.cb * ub + (sg.cdt * dt) * L;   // Eq.7 lines 2, 3 :112-114
-    return L;                                                      // form 3: L itself (mf_eval_L)
-}
-
 template <int EK>
 __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds)
 {

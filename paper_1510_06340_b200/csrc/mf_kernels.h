@@ -3,7 +3,23 @@
 #pragma once
 #include "mf_types.h"
 
+#include <atomic>
+
 namespace mf {
+
+// "once per DEVICE" for function attributes (cudaFuncSetAttribute applies to the current device only): first() is true the first time it is
+// called with a given device current, in any thread.
+struct DeviceOnce {
+    std::atomic<unsigned long long> done[4];      // one bit per device ordinal, 256 devices
+    DeviceOnce() { for (auto& d : done) d.store(0ull); }
+    bool first()
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 256) return true;
+        const unsigned long long bit = 1ull << (dev & 63);
+        return (done[dev >> 6].fetch_or(bit) & bit) == 0;
+    }
+};
 
 // a2: CFL reduction of `U` into ds->smax_bits / ds->status (accumulator must have been reset by begin_step of the previous step or by reset_smax)
 int launch_cfl(const Grid& g, const Eos& q, CState5 U, StepState* ds, int num_sms, cudaStream_t st);
@@ -45,7 +61,7 @@ int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st);    
 int launch_con2prim(const Grid& g, const Eos& q, CState5 U, State5 P, cudaStream_t st); // Eq.23
 int launch_totals(const Grid& g, CState5 U, double* partials /* 5*nblocks */, int nblocks, cudaStream_t st);
 
-// ---- FP64 pipe micro-benchmarks (mf_probe_fp64)
-int probe_fp64(double out[7]);
+// ---- FP64 pipe micro-benchmarks (mf_probe_fp64; diagnostic, not on the hot path)
+int probe_fp64(double out[8]);
 
 } // namespace mf

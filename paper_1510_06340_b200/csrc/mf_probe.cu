@@ -10,9 +10,9 @@ constexpr int CH = 8;
 template <int OP>
 __global__ void __launch_bounds__(256) k_probe(double* out, int iters, double seed, long long* cycles)
 {
-    double x[CH];
+    double x[CH], y[CH], z[CH];
 #pragma unroll
-    for (int c = 0; c < CH; ++c) x[c] = seed + 1e-3 * (threadIdx.x + c);
+    for (int c = 0; c < CH; ++c) { x[c] = seed + 1e-3 * (threadIdx.x + c); y[c] = 1.0 + 1e-9 * (threadIdx.x + c) * seed; z[c] = 1e-9 * (threadIdx.x - c) * seed; }
     const double a = 1.0 + 1e-9, b = 1e-9;
     long long t0 = clock64();
     for (int it = 0; it < iters; ++it) {
@@ -23,12 +23,13 @@ __global__ void __launch_bounds__(256) k_probe(double* out, int iters, double se
             if (OP == 2) x[c] = x[c] * a;
             if (OP == 3) x[c] = 1.0 / (x[c] + 0.5);
             if (OP == 4) x[c] = sqrt(x[c] + 2.0);
+            if (OP == 5) x[c] = fma(y[c], z[c], x[c]);   // three distinct register operands: the register file needs 3 cycles for them
         }
     }
     long long t1 = clock64();
     double s = 0.0;
 #pragma unroll
-    for (int c = 0; c < CH; ++c) s += x[c];
+    for (int c = 0; c < CH; ++c) s += x[c] + (OP == 5 ? y[c] + z[c] : 0.0);
     if (s == 123.456) out[0] = s;             // keeps the loop alive
     if (blockIdx.x == 0 && threadIdx.x == 0 && cycles) *cycles = t1 - t0;
 }
@@ -55,7 +56,7 @@ static double run_probe(int sms, int iters, double* d_out, long long* d_cyc, dou
     return (double)grid * 256.0 * CH * (double)iters / (ms * 1e-3);
 }
 
-int probe_fp64(double out[7])
+int probe_fp64(double out[8])
 {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -1;
@@ -73,6 +74,7 @@ int probe_fp64(double out[7])
     out[4] = run_probe<4>(sms, 1 << 11, d_out, d_cyc, nullptr);
     out[5] = hz;
     out[6] = (double)sms;
+    out[7] = run_probe<5>(sms, 1 << 14, d_out, d_cyc, nullptr);
     cudaFree(d_out); cudaFree(d_cyc);
     return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }

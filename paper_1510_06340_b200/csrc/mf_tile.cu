@@ -12,6 +12,7 @@
 // Face states, fluxes and flux differences never touch HBM.  Three CTAs per SM (24 warps) run out of phase with one another.
 // Arithmetic per cell and per interface is the staged path's, in the same order: the strict build stays bit-identical to the oracle.
 #include "mf_kernels.h"
+#include "mf_blocks.cuh"
 #include <cuda/barrier>
 #include <cstring>
 
@@ -24,27 +25,6 @@ constexpr int TX = 32;               // tile cells along x
 constexpr int TY = 7;                // tile cells along y
 constexpr int NFX = (TX + 1) * TY;   // x interface tasks = 231
 constexpr int NCX = (TX + 2) * TY;   // x cell parts      = 238
-
-__device__ __forceinline__ double jet_source_t(const Grid& g, const Source& s, int i, int j, int k, double t)
-{
-    double x = (i + 0.5 - g.n[0] / 2.0) * g.dx - (s.x0 + t);
-    double y = (j + 0.5 - g.n[1] / 2.0) * g.dx - s.y0;
-    double z = (k + 0.5 - g.n[2] / 2.0) * g.dx - s.z0;
-    double r2 = x * x + y * y + z * z;
-    double arg = -r2 * s.inv_two_s2;
-#ifndef MF_STRICT
-    if (arg < -100.0) return 0.0;            // as in mf_blocks.cuh: below e^-100 of the peak the source is taken as zero
-#endif
-    return s.dEdx * s.norm * exp(arg);
-}
-
-__device__ __forceinline__ double rk_form_t(const Stage& sg, double ua, double ub, double dt, double L)
-{
-    if (sg.form == 0) return ua + dt * L;
-    if (sg.form == 1) return 0.5 * (ua + ub + dt * L);
-    if (sg.form == 2) return sg.ca * ua + sg.cb * ub + (sg.cdt * dt) * L;
-    return L;
-}
 
 // Evolved face states along one axis of the cell at offset o0 (neighbours at om, op; delta at pe in the extended layout):
 // lo = U - s/2 + delta, hi = U + s/2 + delta  (Eq.12, Eq.15-17, Eq.13).  Offsets already carry the boundary mapping (a1).
@@ -238,7 +218,7 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
                 const int kc = kk - 1;
                 const long long o = co + (long long)kc * ns2;
                 double S = 0.0;
-                if (src.on) S = jet_source_t(g, src, gx, gy, kc, ds->t + sg.ts * dt);
+                if (src.on) S = jet_source(g, src, gx, gy, kc, ds->t + sg.ts * dt);
                 double ua5[5], ub5[5];                                   // loaded before the first store (`out` may alias them for all the compiler knows)
 #pragma unroll
                 for (int v = 0; v < 5; ++v) {
@@ -254,7 +234,7 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
                     double L = -acc * g.inv_dx;
 #endif
                     if (src.on && v < 2) L = L + S;
-                    out.q[v][o] = rk_form_t(sg, ua5[v], ub5[v], dt, L);
+                    out.q[v][o] = rk_form(sg, ua5[v], ub5[v], dt, L);
                 }
             }
 #pragma unroll
@@ -295,8 +275,8 @@ int launch_tile_stage(const Grid& g, const Eos& q, int limiter, int predictor, i
     const size_t smem = sizeof(double) * 35 * NT;
     Faces none; memset(&none, 0, sizeof(none));
 #define MF_CASE(L) case L: { \
-        static bool attr_set = false; \
-        if (!attr_set) { cudaFuncSetAttribute(k_tile_stage<L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; } \
+        static DeviceOnce once; \
+        if (once.first()) cudaFuncSetAttribute(k_tile_stage<L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
         k_tile_stage<L, false><<<grid, NT, smem, st>>>(g, q, predictor, k, TZ, ntx, nty, V, D, none, sg, Ua, out, src, ds); } break;
     switch (limiter) {
         MF_CASE(LIM_NONE) MF_CASE(LIM_MINMOD) MF_CASE(LIM_SUPERBEE) MF_CASE(LIM_VANALBADA) MF_CASE(LIM_VANLEER) MF_CASE(LIM_MC) MF_CASE(LIM_FIRST)
@@ -314,8 +294,8 @@ int launch_tile_stage_pre(const Grid& g, const Eos& q, int k, Faces fc, CState5 
     const int TZ = tile_chunk(g, ntx, nty, num_sms);
     const unsigned int grid = (unsigned int)(ntx * nty * ((g.n[2] + TZ - 1) / TZ));
     const size_t smem = sizeof(double) * 35 * NT;
-    static bool attr_set = false;
-    if (!attr_set) { cudaFuncSetAttribute(k_tile_stage<LIM_NONE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
+    static DeviceOnce once;
+    if (once.first()) cudaFuncSetAttribute(k_tile_stage<LIM_NONE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k_tile_stage<LIM_NONE, true><<<grid, NT, smem, st>>>(g, q, 0, k, TZ, ntx, nty, V, V, fc, sg, Ua, out, src, ds);
     return 1;
 }

@@ -52,6 +52,30 @@ def test_batch_of_events_follows_the_oracle_event_by_event(rk, limiter, k):
     np.testing.assert_allclose(g.totals(), sum(g.totals(ev) for ev in range(3)), rtol=1e-12)
 
 
+def test_config4_batch_of_8_full_size_events_against_their_oracles():
+    """BASELINE.json config 4 at full size: the first eight of the 32 seeded 128^3 events in ONE batch (the launch configuration
+    `bench.py --config 4 --batch 8` times), 25 steps, every event compared cell by cell with its own oracle run (own S_max, own dt)."""
+    events = [w.lumpy_event(event=ev) for ev in range(8)]
+    nz, ny, nx = events[0]["shape"]
+    kw = dict(events[0]["scheme"])
+    g = MustaForce(nx, ny, nz, dx=events[0]["dx"], batch=8, **kw)
+    g.set_state(*stack(events))
+    g.step(25, events[0]["cfl"])
+    got = g.get_state()
+    assert g.last_status == 0
+    worst = 0.0
+    for ev, st in enumerate(events):
+        o = Oracle(nx, ny, nz, dx=st["dx"], omp=True, **kw)
+        o.set_state(*[st[f] for f in FIELDS])
+        o.step(25, st["cfl"])
+        r = parity.assert_parity([a[ev] for a in got], o.get_state(), what="config 4 event %d of a batch of 8 at 128^3" % ev)
+        worst = max(worst, max(r))
+        t, dt, steps = g.time(ev)
+        to, dto, _ = o.time()
+        assert steps == 25 and t == pytest.approx(to, rel=1e-12) and dt == pytest.approx(dto, rel=1e-12)
+    print("config 4, 8 events at 128^3, 25 steps: worst rel diff", worst)
+
+
 def test_batch_equals_single_contexts_bit_for_bit():
     """Same kernels, same arithmetic: an event inside a batch gives the bits it gives in a context of its own (fixed dt and CFL mode)."""
     shape = (12, 16, 20)
