@@ -46,6 +46,7 @@ def _load(omp):
         "mfo_set_boundary": (C.c_int, [vp, C.c_int]),
         "mfo_set_cs2": (C.c_int, [vp, C.c_double]),
         "mfo_set_predictor": (C.c_int, [vp, C.c_int]),
+        "mfo_set_state_precision": (C.c_int, [vp, C.c_int]),
         "mfo_set_alpha": (C.c_int, [vp, C.c_double]),
         "mfo_set_jet_source": (C.c_int, [vp] + [C.c_double] * 5),
         "mfo_set_eos_table": (C.c_int, [vp, C.c_int, C.c_int] + [C.c_double] * 4 + [_dp]),
@@ -87,7 +88,7 @@ class Oracle:
     """One oracle context.  Arrays are numpy float64 of shape (nz, ny, nx) (x fastest) or flat."""
 
     def __init__(self, nx, ny=1, nz=1, dx=1.0, limiter="minmod", k_stages=2, rk=2, bc="outflow",
-                 predictor=True, alpha=None, cs2=None, omp=False, eos_table=None):
+                 predictor=True, alpha=None, cs2=None, omp=False, eos_table=None, state_bits=64):
         self.lib = _load(omp)
         self.shape = (nz, ny, nx)
         self.n = nx * ny * nz
@@ -104,6 +105,8 @@ class Oracle:
             self._chk(self.lib.mfo_set_cs2(self.h, float(cs2)))
         if eos_table is not None:
             self.set_eos_table(eos_table)
+        if state_bits != 64:
+            self._chk(self.lib.mfo_set_state_precision(self.h, int(state_bits)))
 
     def _chk(self, rc, allow=()):
         if rc != OK and rc not in allow:

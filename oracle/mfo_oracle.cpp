@@ -26,6 +26,9 @@
  * sequence; tests/test_oracle_pieces.py::test_musta_linear_flux_closed_form), the signal speed at rest / at
  * |v| -> 1 / as a sum of rapidities, and the source's RK stage times as the nodes of the trapezoidal and
  * Simpson rules on a one-cell grid (error orders dt^3, dt^5 against the exact erf integral).
+ * Single-precision state mode (mfo_set_state_precision, reading A19): tests/test_oracle_state32.py - stored values are
+ * floats, one step equals Eq.6 / Eq.7 composed in numpy with float32 rounding of every stage around the 64-bit mfo_eval_L, uniform
+ * state fixed, conservation and distance to the 64-bit run at single-precision round-off.
  * PARITY UNPINNED by the paper (definitions of ours): accuracy effect of running the
  * Hancock half step inside every RK stage (A4), admissibility-guard constants (A12), jet source
  * definition (A14), charge profile (A13).
@@ -261,6 +264,7 @@ struct mfo_ctx {
     std::vector<double> table;   /* owned copy of ln p for the tabulated EOS */
     double alpha;
     double jet_dEdx, jet_sigma, jet_x0[3];
+    int state_bits;      /* 64 (default) or 32: every STORED state value is rounded to float (reading A19) */
     double t, last_dt;
     long long steps;
     int status;
@@ -428,7 +432,7 @@ void rk_combine(mfo_ctx* c, std::vector<double> out[5], double ca, const std::ve
                     if (form == 0)      r = Ua[q][o] + cdt * Lq;                                   /* U + dt L          */
                     else if (form == 1) r = 0.5 * (Ua[q][o] + Ub[q][o] + cdt * Lq);               /* Eq.6 second line  */
                     else                r = ca * Ua[q][o] + cb * Ub[q][o] + cdt * Lq;             /* Eq.7 lines 2, 3   */
-                    out[q][o] = r;
+                    out[q][o] = c->state_bits == 32 ? (double)(float)r : r;                        /* A19: the stored state is single precision */
                 }
             }
 }
@@ -460,6 +464,16 @@ double max_signal_speed(mfo_ctx* c, int* bad)
     }
     if (bad) *bad = nbad;
     return smax;
+}
+
+/* A19 ("The state of the system is saved as 5 single precision floating-point numbers per lattice cell"): in 32-bit state
+ * mode every value that is STORED as a state - the state handed in, and the result of every Runge-Kutta stage - is rounded to float
+ * (round to nearest even); all arithmetic between a load and the next store stays double. */
+void round_stored_state(mfo_ctx* c)
+{
+    if (c->state_bits != 32) return;
+    for (int q = 0; q < 5; ++q)
+        for (long o = 0; o < c->ncell; ++o) c->U[q][o] = (double)(float)c->U[q][o];
 }
 
 void one_step(mfo_ctx* c, double dt)
@@ -507,6 +521,7 @@ mfo_ctx* mfo_create(int nx, int ny, int nz, double dx, int eos, int limiter, int
     c->rk = 2; c->bc = MFO_BC_OUTFLOW; c->predictor = 1;
     c->P.cs2 = 1.0 / 3.0; c->P.kind = 0; c->P.ne = c->P.nn = 0; c->P.ln_e0 = c->P.dln_e = c->P.n0 = c->P.dn = 0.0; c->P.lnp = nullptr;
     c->alpha = c->nact > 0 ? (double)c->nact : 1.0;         /* A9: alpha = number of active directions */
+    c->state_bits = 64;
     c->jet_dEdx = 0.0; c->jet_sigma = 1.0; c->jet_x0[0] = c->jet_x0[1] = c->jet_x0[2] = 0.0;
     c->t = 0.0; c->last_dt = 0.0; c->steps = 0; c->status = MFO_OK;
     try {
@@ -529,6 +544,7 @@ int mfo_set_state(mfo_ctx* c, const double* E, const double* Mx, const double* M
     if (!E || !Mx || !My || !Mz || !R) return fail(c, MFO_EINVAL, "null pointer");
     const double* src[5] = { E, Mx, My, Mz, R };
     for (int q = 0; q < 5; ++q) std::memcpy(c->U[q].data(), src[q], sizeof(double) * c->ncell);
+    round_stored_state(c);
     c->t = 0.0; c->last_dt = 0.0; c->steps = 0; c->status = MFO_OK;
     return MFO_OK;
 }
@@ -573,6 +589,7 @@ int mfo_set_state_prim(mfo_ctx* c, const double* e, const double* vx, const doub
         mfo_prim2con(c, prim, U);
         for (int q = 0; q < 5; ++q) c->U[q][o] = U[q];
     }
+    round_stored_state(c);
     c->t = 0.0; c->last_dt = 0.0; c->steps = 0; c->status = MFO_OK;
     return MFO_OK;
 }
@@ -645,6 +662,14 @@ int mfo_get_time(mfo_ctx* c, double* t, double* last_dt, long long* steps)
 int mfo_set_rk(mfo_ctx* c, int order) { if (!c) return MFO_EINVAL; if (order != 2 && order != 3) return fail(c, MFO_EINVAL, "rk order must be 2 or 3"); c->rk = order; return MFO_OK; }
 int mfo_set_boundary(mfo_ctx* c, int bc) { if (!c) return MFO_EINVAL; if (bc != MFO_BC_OUTFLOW && bc != MFO_BC_PERIODIC) return fail(c, MFO_EINVAL, "unknown bc"); c->bc = bc; return MFO_OK; }
 int mfo_set_cs2(mfo_ctx* c, double cs2) { if (!c) return MFO_EINVAL; if (!(cs2 > 0.0) || !(cs2 < 1.0)) return fail(c, MFO_EINVAL, "cs2 must be in (0,1)"); c->P.cs2 = cs2; return MFO_OK; }
+int mfo_set_state_precision(mfo_ctx* c, int bits)
+{
+    if (!c) return MFO_EINVAL;
+    if (bits != 32 && bits != 64) return fail(c, MFO_EINVAL, "state precision must be 32 or 64 bits");
+    c->state_bits = bits;
+    round_stored_state(c);
+    return MFO_OK;
+}
 int mfo_set_predictor(mfo_ctx* c, int on) { if (!c) return MFO_EINVAL; c->predictor = on ? 1 : 0; return MFO_OK; }
 int mfo_set_alpha(mfo_ctx* c, double alpha) { if (!c) return MFO_EINVAL; if (!(alpha > 0.0)) return fail(c, MFO_EINVAL, "alpha must be > 0"); c->alpha = alpha; return MFO_OK; }
 int mfo_set_jet_source(mfo_ctx* c, double dEdx, double sigma, double x0, double y0, double z0)

@@ -45,6 +45,9 @@ int mfo_set_rk(mfo_ctx*, int order);
 int mfo_set_boundary(mfo_ctx*, int bc);
 int mfo_set_cs2(mfo_ctx*, double cs2);
 int mfo_set_predictor(mfo_ctx*, int on);
+/* 32: the stored state is single precision as in the paper's own code (reading A19) - the state handed in and the
+ * result of every Runge-Kutta stage are rounded to float, arithmetic stays double.  64 (default): no rounding.  Rounds the current state. */
+int mfo_set_state_precision(mfo_ctx*, int bits);
 int mfo_set_alpha(mfo_ctx*, double alpha);
 int mfo_set_jet_source(mfo_ctx*, double dEdx, double sigma, double x0, double y0, double z0);
 /* tabulated EOS (context created with MFO_EOS_TABLE): ln p on a grid uniform in ln e (ne points) and in n (nn points, e fastest) */
