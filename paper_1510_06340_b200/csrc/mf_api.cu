@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -40,6 +41,7 @@ struct mf_ctx {
     double* table;           // tabulated EOS: ln p, device copy
     int smax_valid;          // the device-side S_max accumulator already holds the reduction of the current U^n (fused into the last combine)
     StepState* ds;           // one per event
+    StepConst* dsc;          // the step's multipliers per event: source of the constant-memory copy (mf_stepconst.cuh)
     StepState* h_ds;         // pinned mirror
     double* partials;        // totals: 5*nblocks doubles
     double* h_partials;
@@ -65,6 +67,29 @@ struct mf_ctx {
 namespace {
 
 thread_local std::string g_create_err;
+
+// Constant-memory slots for the step scalars (MF_CSLOTS events over all live contexts): first fit over a bitmap; -1 when nothing fits,
+// the context then reads the scalars from global memory.
+std::mutex g_slot_mutex;
+bool g_slot_used[MF_CSLOTS];
+int slots_acquire(int n)
+{
+    if (n > MF_CSLOTS) return -1;
+    std::lock_guard<std::mutex> lock(g_slot_mutex);
+    for (int b = 0; b + n <= MF_CSLOTS; ++b) {
+        int i = 0;
+        while (i < n && !g_slot_used[b + i]) ++i;
+        if (i == n) { for (i = 0; i < n; ++i) g_slot_used[b + i] = true; return b; }
+        b += i;
+    }
+    return -1;
+}
+void slots_release(int b, int n)
+{
+    if (b < 0) return;
+    std::lock_guard<std::mutex> lock(g_slot_mutex);
+    for (int i = 0; i < n; ++i) g_slot_used[b + i] = false;
+}
 
 int fail(mf_ctx* c, int code, const std::string& msg) { if (c) c->err = msg; else g_create_err = msg; return code; }
 
@@ -371,8 +396,10 @@ mf_ctx* mf_create_batch(int nevents, int nx, int ny, int nz, double dx, int eos,
     mf_ctx* c = new (std::nothrow) mf_ctx();
     if (!c) { fail(nullptr, MF_ENOMEM, "host allocation failed"); return nullptr; }
     memset(&c->g, 0, sizeof(c->g));
+    c->g.cslot = -1;
+    c->nev = 0;
     c->U[0] = c->U[1] = c->U[2] = nullptr; c->faces = c->fluxes = nullptr; c->delta = nullptr;
-    c->ds = nullptr; c->h_ds = nullptr;
+    c->ds = nullptr; c->h_ds = nullptr; c->dsc = nullptr;
     c->partials = nullptr; c->h_partials = nullptr; c->own_stream = nullptr; c->stream = nullptr;
     cudaGetDevice(&c->dev);
     cudaDeviceProp prop;
@@ -401,6 +428,7 @@ mf_ctx* mf_create_batch(int nevents, int nx, int ny, int nz, double dx, int eos,
     g.es[0] = 1; g.es[1] = g.e[0]; g.es[2] = (long long)g.e[0] * g.e[1];
     g.dx = dx;
     g.inv_dx = 1.0 / dx;
+    g.cslot = slots_acquire(nevents);
     for (int a = 0; a < 2; ++a) for (int m = 0; m < 3; ++m) g.dv[a][m] = make_fastdiv((unsigned int)(n[a] + m));
     set_eos(c->q, 1.0 / 3.0);
     clear_table(c->q);
@@ -419,6 +447,7 @@ mf_ctx* mf_create_batch(int nevents, int nx, int ny, int nz, double dx, int eos,
     c->stream = c->own_stream;
     for (int r = 0; ok && r < 3; ++r) ok = cudaMalloc(&c->U[r], sizeof(double) * 5 * c->nst) == cudaSuccess;
     ok = ok && cudaMalloc(&c->ds, sizeof(StepState) * nevents) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->dsc, sizeof(StepConst) * nevents) == cudaSuccess;
     ok = ok && cudaMallocHost(&c->h_ds, sizeof(StepState) * nevents) == cudaSuccess;
     ok = ok && cudaMalloc(&c->partials, sizeof(double) * 5 * c->nblocks_tot) == cudaSuccess;
     ok = ok && cudaMallocHost(&c->h_partials, sizeof(double) * 5 * c->nblocks_tot) == cudaSuccess;
@@ -446,6 +475,8 @@ void mf_destroy(mf_ctx* c)
     if (c->delta) cudaFree(c->delta);
     if (c->table) cudaFree(c->table);
     if (c->ds) cudaFree(c->ds);
+    if (c->dsc) cudaFree(c->dsc);
+    slots_release(c->g.cslot, c->nev);
     if (c->h_ds) cudaFreeHost(c->h_ds);
     if (c->partials) cudaFree(c->partials);
     if (c->h_partials) cudaFreeHost(c->h_partials);
@@ -609,6 +640,16 @@ int mf_get_state_prim(mf_ctx* c, double* e, double* vx, double* vy, double* vz, 
     return fetch_step_state(c);
 }
 
+// per-step scalars on the device, then their copy into the constant memory of the unit whose kernels run this path
+static int begin_step(mf_ctx* c, int mode, double value)
+{
+    c->launches += launch_begin_step(c->ds, c->dsc, c->nev, mode, value, c->g.dx, c->alpha, c->stream);
+    if (c->g.cslot >= 0 && (c->path == MF_PATH_STAGED || c->path == MF_PATH_HYBRID)) {
+        if (upload_step_const_staged(c->dsc, c->g.cslot, c->nev, c->stream) != 0) { cudaGetLastError(); return fail(c, MF_ECUDA, "copy of the step scalars to constant memory failed"); }
+    }
+    return MF_OK;
+}
+
 // ---- stepping.  One step = (CFL reduction if the accumulator is stale) + per-step scalars + the RK stages; nothing in it needs the host.
 // mode 0: dt = value*dx/S_max (value = cfl); mode 1: dt = value.
 static int enqueue_step(mf_ctx* c, int mode, double value)
@@ -618,7 +659,8 @@ static int enqueue_step(mf_ctx* c, int mode, double value)
         c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->nst), c->ds, c->num_sms, c->stream);   // a2, from U^n
         prof_end(c, ps);
     }
-    c->launches += launch_begin_step(c->ds, c->nev, mode, value, c->g.dx, c->alpha, c->stream);
+    int rc = begin_step(c, mode, value);
+    if (rc != MF_OK) return rc;
     return run_step(c);
 }
 
@@ -718,7 +760,7 @@ int mf_eval_L(mf_ctx* c, double dt, double* L_E, double* L_Mx, double* L_My, dou
     if (!(dt > 0.0) || !L_E || !L_Mx || !L_My || !L_Mz || !L_R) return fail(c, MF_EINVAL, "bad dt or null pointer");
     double* Un = c->U[c->cur];
     double* scratch = c->U[(c->cur + 1) % c->nreg];
-    c->launches += launch_begin_step(c->ds, c->nev, 1, dt, c->g.dx, c->alpha, c->stream);
+    { int rb = begin_step(c, 1, dt); if (rb != MF_OK) return rb; }
     Stage sg = { 3, 0.0, 0.0, 0.0, 0.0 };
     c->smax_valid = 0;
     Source keep = c->src;

@@ -418,7 +418,7 @@ __device__ __forceinline__ bool flux_fast(const Eos& q, const double (&U)[5], do
     // The words are compared as UNSIGNED numbers with one unit of room (the high word of |M|^2 at least TWO below that of E^2): a NaN of
     // either sign in M (CUDA's canonical NaN has the sign bit set) is larger than every finite E^2 and fails the test.
     const bool ok = (__double2hiint(E) > 0x3D719799) && ((unsigned int)__double2hiint(M2) + 1u < (unsigned int)__double2hiint(EE));
-    const double Qh = sqrt_pos(fma(-q.cs2, M2, q.qc1sq * EE));
+    const double Qh = sqrt_pos(fma(q.cs2, -M2, q.qc1sq * EE));      // (the sign on the register operand: cs2 stays a uniform-register operand)
     double y;
     {
         const double x = fma(q.hc1, E, Qh);
@@ -452,10 +452,18 @@ __device__ __forceinline__ void flux_eval(const Eos& q, const double (&U)[5], do
 
 // ---- MUSTA_k with FORCE-alpha, steps 1-5 :123-135, Eq.8-11 :130-149 (A1: Richtmyer state uses the flux difference)
 // A, B are U_L^(0), U_R^(0) on entry and are overwritten.
+// The stage coefficients: lam, c_lw = alpha lam/2, c_lf = 1/(2 alpha lam) as the step computed them (A16), and the negated multiples the
+// product form multiplies with.  Taken from constant memory they are uniform-register operands (mf_stepconst.cuh).
+struct MustaCoef {
+    double lam, c_lw, c_lf;
+    double nc_lw, nc2_lf, nhlam;      // -c_lw, -2 c_lf, -lam/2
+};
+
 template <int D, int EK = 0>
-__device__ __forceinline__ void musta_flux(const Eos& q, int k, double lam, double c_lw, double c_lf,
-                                           double (&A)[5], double (&B)[5], double (&F)[5])
+__device__ __forceinline__ void musta_flux(const Eos& q, int k, const MustaCoef& mc, double (&A)[5], double (&B)[5], double (&F)[5])
 {
+    const double lam = mc.lam, c_lw = mc.c_lw, c_lf = mc.c_lf;
+    (void)lam; (void)c_lw; (void)c_lf;
 #ifndef MF_STRICT
     if (EK == 0) {
     // The same stages on the mean s = (A+B)/2 and the half jump d = (B-A)/2 of the two states, with the constant factors folded:
@@ -463,7 +471,9 @@ __device__ __forceinline__ void musta_flux(const Eos& q, int k, double lam, doub
     //   Eq.9,11  2F = F^lw + (F_A + F_B)/2 - 2 c_lf d
     //   Eq.8   s' = s - (lam/2)(F_B - F_A),   d' = d - (lam/2)(F_A + F_B - 2F)
     // 10 FP64 instructions per component and stage (6 in the last) instead of 13 (9), and the 24-instruction flux.
-    const double c2_lf = 2.0 * c_lf, hlam = 0.5 * lam;
+    // Every multiplier below is one of mc's scalars, so that each DFMA reads at most two registers (a DFMA with three distinct register
+    // operands holds the FP64 pipe for 3 cycles instead of 2).
+    const double nc_lw = mc.nc_lw, nc2_lf = mc.nc2_lf, nhlam = mc.nhlam;
     double s[5], d[5];
 #pragma unroll
     for (int c = 0; c < 5; ++c) { s[c] = 0.5 * (A[c] + B[c]); d[c] = 0.5 * (B[c] - A[c]); }
@@ -477,16 +487,16 @@ __device__ __forceinline__ void musta_flux(const Eos& q, int k, double lam, doub
             const double FD = FB[c] - FA[c];
             FA[c] = FA[c] + FB[c];                                                            // F_A + F_B from here on
             FB[c] = FD;                                                                       // F_B - F_A from here on
-            W[c] = fma(-c_lw, FD, s[c]);                                                      // Eq.10
+            W[c] = fma(nc_lw, FD, s[c]);                                                      // Eq.10
         }
         if (!flux_fast<D>(q, W, F)) flux_d<D>(q, W, F);                                       // F^lw
 #pragma unroll
-        for (int c = 0; c < 5; ++c) F[c] = fma(-c2_lf, d[c], fma(0.5, FA[c], F[c]));          // 2F: Eq.9 with Eq.11 inside
+        for (int c = 0; c < 5; ++c) F[c] = fma(nc2_lf, d[c], fma(0.5, FA[c], F[c]));          // 2F: Eq.9 with Eq.11 inside
         if (l == k) break;
 #pragma unroll
         for (int c = 0; c < 5; ++c) {                                                         // Eq.8
-            s[c] = fma(-hlam, FB[c], s[c]);
-            d[c] = fma(-hlam, FA[c] - F[c], d[c]);
+            s[c] = fma(nhlam, FB[c], s[c]);
+            d[c] = fma(nhlam, FA[c] - F[c], d[c]);
             A[c] = s[c] - d[c];
             B[c] = s[c] + d[c];
         }

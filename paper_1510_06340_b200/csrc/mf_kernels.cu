@@ -3,6 +3,7 @@
 // prim<->con conversions, totals.  Boundary handling (a1) is index mapping in the loads: no stored ghosts.
 #include "mf_kernels.h"
 #include "mf_blocks.cuh"
+#include "mf_stepconst.cuh"
 
 namespace mf {
 
@@ -62,11 +63,12 @@ int launch_cfl(const Grid& g, const Eos& q, CState5 U, StepState* ds, int num_sm
 
 // =========================================================================== per-step scalars
 // one thread per event of the batch
-__global__ void k_begin_step(StepState* ds, int nev, int mode, double value, double dx, double alpha)
+__global__ void k_begin_step(StepState* ds, StepConst* dsc, int nev, int mode, double value, double dx, double alpha)
 {
     const int ev = blockIdx.x * blockDim.x + threadIdx.x;
     if (ev >= nev) return;
     ds += ev;
+    dsc += ev;
     double dt;
     if (mode == 0) {
         double smax = __longlong_as_double((long long)ds->smax_bits);
@@ -81,6 +83,9 @@ __global__ void k_begin_step(StepState* ds, int nev, int mode, double value, dou
     ds->c_lw = 0.5 * alpha * lam;                                 // A16: computed once per step, in this order
     ds->c_lf = 0.5 / (alpha * lam);
     ds->smax_bits = 0ull;
+    // the same scalars, with the negated multiples of the product build's MUSTA, for the constant-memory copy (mf_stepconst.cuh)
+    dsc->dt = dt; dsc->lam = lam; dsc->hl = ds->hl; dsc->c_lw = ds->c_lw; dsc->c_lf = ds->c_lf;
+    dsc->nc_lw = -ds->c_lw; dsc->nc2_lf = -2.0 * ds->c_lf; dsc->nhlam = -0.5 * lam;
 }
 
 __global__ void k_end_step(StepState* ds, int nev)
@@ -101,17 +106,18 @@ __global__ void k_reset(StepState* ds, int nev)
     ds->smax_bits = 0ull; ds->status = 0; ds->pad = 0; ds->steps = 0;
 }
 
-int launch_begin_step(StepState* ds, int nev, int mode, double value, double dx, double alpha, cudaStream_t st)
+int launch_begin_step(StepState* ds, StepConst* dsc, int nev, int mode, double value, double dx, double alpha, cudaStream_t st)
 {
-    k_begin_step<<<(nev + 63) / 64, nev < 64 ? nev : 64, 0, st>>>(ds, nev, mode, value, dx, alpha);
+    k_begin_step<<<(nev + 63) / 64, nev < 64 ? nev : 64, 0, st>>>(ds, dsc, nev, mode, value, dx, alpha);
     return 1;
 }
+int upload_step_const_staged(const StepConst* dsc, int slot, int nev, cudaStream_t st) { return upload_step_const(dsc, slot, nev, st); }
 int launch_end_step(StepState* ds, int nev, cudaStream_t st) { k_end_step<<<(nev + 63) / 64, nev < 64 ? nev : 64, 0, st>>>(ds, nev); return 1; }
 int launch_reset(StepState* ds, int nev, cudaStream_t st) { k_reset<<<(nev + 63) / 64, nev < 64 ? nev : 64, 0, st>>>(ds, nev); return 1; }
 
 // =========================================================================== a3 + a4: cell stage
 // One thread per cell of the extended region (interior + 1 layer on every active axis).
-template <int LIM, int EK>
+template <int LIM, int EK, bool UC>
 __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, int predictor, CState5 V, Faces fc, State5 Wout, const StepState* ds)
 {
     // linear index over the extended region, x fastest: 256 consecutive cells per block (measured on B200: 32 x 8 tiles, which
@@ -129,7 +135,6 @@ __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, 
     const unsigned int ns[3] = { (unsigned int)g.ns[0], (unsigned int)g.ns[1], (unsigned int)g.ns[2] };
     const unsigned int o0 = blockIdx.y * (unsigned int)g.ncell + cc[0] * ns[0] + cc[1] * ns[1] + cc[2] * ns[2];
     const unsigned int pu = blockIdx.y * (unsigned int)g.next + (unsigned int)p;
-    ds += blockIdx.y;
     double U0[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) U0[v] = V.q[v][o0];
@@ -162,7 +167,7 @@ __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, 
         }
     }
     if (predictor) {                                                        // Eq.13 (A3)
-        const double hl = ds->hl;
+        const double hl = step_scalars<UC>(g, ds).hl;
         double delta[5];
         bool first = true;
         double Fl[5], Fr[5];
@@ -227,7 +232,7 @@ __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, 
 #pragma unroll
     for (int v = 0; v < 5; ++v) W[v] = U0[v];
     if (predictor) {                                                        // Eq.13 (A3)
-        const double hl = ds->hl;
+        const double hl = step_scalars<UC>(g, ds).hl;
         double acc[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
         double UL[5], UR[5], Fl[5], Fr[5];
         if (g.act[0]) {
@@ -265,8 +270,9 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
     State5 Wout;
     for (int v = 0; v < 5; ++v) Wout.q[v] = fc.f[g.act[0] ? 0 : (g.act[1] ? 1 : 2)][1][v];
     switch (limiter) {
-#define MF_CASE(L) case L: if (q.kind) k_cell_stage<L, 1><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); \
-                           else k_cell_stage<L, 0><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); break;
+#define MF_CASE(L) case L: if (q.kind) k_cell_stage<L, 1, false><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); \
+                           else if (g.cslot >= 0) k_cell_stage<L, 0, true><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); \
+                           else k_cell_stage<L, 0, false><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); break;
         MF_CASE(LIM_NONE) MF_CASE(LIM_MINMOD) MF_CASE(LIM_SUPERBEE) MF_CASE(LIM_VANALBADA) MF_CASE(LIM_VANLEER) MF_CASE(LIM_MC) MF_CASE(LIM_FIRST)
 #undef MF_CASE
     default: return 0;
@@ -276,7 +282,7 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
 
 // =========================================================================== a5 + a6: interface fluxes
 // One thread per interface between cell c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
-template <int D, int EK>
+template <int D, int EK, bool UC>
 __global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, int k, CState5 Wc, Faces fc, Fluxes fx, const StepState* ds)
 {
     int m[3] = { g.n[0], g.n[1], g.n[2] };
@@ -289,7 +295,6 @@ __global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, 
     c[D] -= 1;
     const unsigned int es[3] = { (unsigned int)g.es[0], (unsigned int)g.es[1], (unsigned int)g.es[2] };
     const unsigned int p = blockIdx.y * (unsigned int)g.next + (c[0] + g.h[0]) * es[0] + (c[1] + g.h[1]) * es[1] + (c[2] + g.h[2]) * es[2];   // < 2^32 (mf_create)
-    ds += blockIdx.y;
     double A[5], B[5], F[5];
 #ifdef MF_STRICT
 #pragma unroll
@@ -301,7 +306,7 @@ __global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, 
         for (int v = 0; v < 5; ++v) { A[v] = Wc.q[v][p] + fc.f[D][0][v][p]; B[v] = Wc.q[v][pn] - fc.f[D][0][v][pn]; }
     }
 #endif
-    musta_flux<D, EK>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
+    musta_flux<D, EK>(q, k, musta_coef(step_scalars<UC>(g, ds)), A, B, F);
 #pragma unroll
     for (int v = 0; v < 5; ++v) fx.f[D][v][p] = F[v];
 }
@@ -316,9 +321,13 @@ int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, F
         long long total = 1;
         for (int a = 0; a < 3; ++a) total *= (a == d) ? g.n[a] + 1 : g.n[a];
         const dim3 nb(blocks_for(total, FT), g.nev);
-        if (d == 0) { if (q.kind) k_flux_stage<0, 1><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); else k_flux_stage<0, 0><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); }
-        if (d == 1) { if (q.kind) k_flux_stage<1, 1><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); else k_flux_stage<1, 0><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); }
-        if (d == 2) { if (q.kind) k_flux_stage<2, 1><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); else k_flux_stage<2, 0><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); }
+#define MF_FLUX(D_) do { if (q.kind) k_flux_stage<D_, 1, false><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); \
+                         else if (g.cslot >= 0) k_flux_stage<D_, 0, true><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); \
+                         else k_flux_stage<D_, 0, false><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds); } while (0)
+        if (d == 0) MF_FLUX(0);
+        if (d == 1) MF_FLUX(1);
+        if (d == 2) MF_FLUX(2);
+#undef MF_FLUX
         ++launches;
     }
     return launches;
@@ -397,7 +406,7 @@ int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua,
 // instead was 40% slower (the 35 KB per block cost the L1 hits of the x-neighbour loads).  History of this kernel: 1.56 -> 1.37 -> 1.03 -> 0.95 ms per launch.
 // FORM (the RK form of the stage) and CFL (last stage of a step) are compile-time: the stage loop has no form branches, and the
 // signal-speed code with its block reduction exists only in the instantiations that need it.
-template <int EK, int FORM, bool CFL>
+template <int EK, int FORM, bool CFL, bool UC>
 __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
                                                           Source src, StepState* ds)
 {
@@ -411,6 +420,7 @@ __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q,
     unsigned int p = 0;                                                      // cell offsets fit 32 bits (mf_create)
     double F[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
     const unsigned int eo = blockIdx.y * (unsigned int)g.ncell, ep = blockIdx.y * (unsigned int)g.next;   // this block's event
+    const StepConst sc = step_scalars<UC>(g, ds);
     ds += blockIdx.y;
     if (live) {
         unflatten3((unsigned int)I, g.dv[0][1], g.dv[1][0], f, j, kz);                       // f: interface between cells f-1 and f of row (j, kz)
@@ -423,7 +433,7 @@ __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q,
 #pragma unroll
         for (int v = 0; v < 5; ++v) { A[v] = fc.f[0][1][v][p] + fc.f[0][0][v][p]; B[v] = fc.f[0][1][v][p + 1] - fc.f[0][0][v][p + 1]; }
 #endif
-        musta_flux<0, EK>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
+        musta_flux<0, EK>(q, k, musta_coef(sc), A, B, F);
     }
     // The combine's operands.  Every one is loaded before the first store: `out` may alias the inputs as far as the compiler knows (and does
     // alias U_(s) in low-storage mode), so loads written after a store would wait for it - five dependent round trips to memory instead of
@@ -447,7 +457,7 @@ __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q,
     double smax = 0.0;
     int bad = 0;
     if (owns_cell) {
-        const double dt = ds->dt;
+        const double dt = sc.dt;
         double S = 0.0;
         if (src.on) S = jet_source(g, src, f, j, kz, ds->t + sg.ts * dt);
         double W[5];
@@ -476,7 +486,8 @@ int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx
 {
     const long long total = (long long)(g.n[0] + 1) * g.n[1] * g.n[2];
     const dim3 nb(blocks_for(total, XT - 1), g.nev);
-#define MF_XFC(EK_, FORM_, CFL_) k_xflux_combine<EK_, FORM_, CFL_><<<nb, XT, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds)
+#define MF_XFC(EK_, FORM_, CFL_) do { if (EK_ == 0 && g.cslot >= 0) k_xflux_combine<EK_, FORM_, CFL_, EK_ == 0><<<nb, XT, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds); \
+                                      else k_xflux_combine<EK_, FORM_, CFL_, false><<<nb, XT, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds); } while (0)
 #define MF_XFC_FORMS(EK_) \
     if (sg.form == 0) { if (sg.cfl) MF_XFC(EK_, 0, true); else MF_XFC(EK_, 0, false); } \
     else if (sg.form == 1) { if (sg.cfl) MF_XFC(EK_, 1, true); else MF_XFC(EK_, 1, false); } \

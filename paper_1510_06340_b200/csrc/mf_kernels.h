@@ -24,7 +24,9 @@ struct DeviceOnce {
 // a2: CFL reduction of `U` into ds->smax_bits / ds->status (accumulator must have been reset by begin_step of the previous step or by reset_smax)
 int launch_cfl(const Grid& g, const Eos& q, CState5 U, StepState* ds, int num_sms, cudaStream_t st);
 // per-step scalars on the device: mode 0: dt = value*dx/smax (cfl), mode 1: dt = value (fixed); resets the smax accumulator
-int launch_begin_step(StepState* ds, int nev, int mode, double value, double dx, double alpha, cudaStream_t st);   // ds: one StepState per event
+int launch_begin_step(StepState* ds, StepConst* dsc, int nev, int mode, double value, double dx, double alpha, cudaStream_t st);   // ds, dsc: one per event
+// copy dsc[0..nev) into the constant-memory step scalars of the translation unit that holds the staged kernels (mf_stepconst.cuh); 0 = ok
+int upload_step_const_staged(const StepConst* dsc, int slot, int nev, cudaStream_t st);
 int launch_end_step(StepState* ds, int nev, cudaStream_t st);
 int launch_reset(StepState* ds, int nev, cudaStream_t st);
 

@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, i
 #pragma unroll
         for (int v = 0; v < 5; ++v) { A[v] = A[v] + __ldg(&Dl.q[v][p]); B[v] = B[v] + __ldg(&Dl.q[v][p + es[D]]); }
     }
-    musta_flux<D, 0>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
+    musta_flux<D, 0>(q, k, musta_coef_of(ds), A, B, F);
 #pragma unroll
     for (int v = 0; v < 5; ++v) fx.f[D][v][p] = F[v];
 }
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int li
 #pragma unroll
             for (int v = 0; v < 5; ++v) { A[v] = A[v] + __ldg(&Dl.q[v][p]); B[v] = B[v] + __ldg(&Dl.q[v][p + 1]); }
         }
-        musta_flux<0, 0>(q, k, ds->lam, ds->c_lw, ds->c_lf, A, B, F);
+        musta_flux<0, 0>(q, k, musta_coef_of(ds), A, B, F);
     }
     // The combine's operands: all loaded before the first store (`out` may alias the inputs as far as the compiler knows: loads written after
     // a store would wait for it - five dependent round trips to memory instead of one), and issued before the barrier, so that their

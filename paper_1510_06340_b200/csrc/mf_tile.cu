@@ -104,7 +104,8 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
     const int x0 = tx * TX, y0 = ty * TY;
     const int z0 = tz * TZ, z1 = min(z0 + TZ, nz);
-    const double dt = ds->dt, lam = ds->lam, c_lw = ds->c_lw, c_lf = ds->c_lf;
+    const double dt = ds->dt;
+    const MustaCoef mcf = musta_coef_of(ds);
     const long long ns2 = g.ns[2], es2 = g.es[2];
 
     // ---- roles of this thread, fixed for the whole march (plane offsets fit in 32 bits)
@@ -178,7 +179,7 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
             double A[5], B[5], F[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) { A[v] = s_Ax[v][t]; B[v] = s_Bx[v][t]; }
-            musta_flux<0>(q, k, lam, c_lw, c_lf, A, B, F);
+            musta_flux<0>(q, k, mcf, A, B, F);
 #pragma unroll
             for (int v = 0; v < 5; ++v) s_Ax[v][t] = F[v];           // only this task reads slot t
         }
@@ -186,7 +187,7 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
             double A[5], B[5], F[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) { A[v] = s_Ay[v][t]; B[v] = s_By[v][t]; }
-            musta_flux<1>(q, k, lam, c_lw, c_lf, A, B, F);
+            musta_flux<1>(q, k, mcf, A, B, F);
 #pragma unroll
             for (int v = 0; v < 5; ++v) s_Ay[v][t] = F[v];
         }
@@ -213,7 +214,7 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
                     else { prefetch_l2(&V.q[v][co + zp2]); prefetch_l2(&Dl.q[v][cpe + (long long)(kk + 2) * es2]); }
                 }
             }
-            musta_flux<2>(q, k, lam, c_lw, c_lf, A, B, F);
+            musta_flux<2>(q, k, mcf, A, B, F);
             if (kk > z0) {                                           // cell (gx, gy, kk-1) is complete
                 const int kc = kk - 1;
                 const long long o = co + (long long)kc * ns2;

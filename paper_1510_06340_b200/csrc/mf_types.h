@@ -39,6 +39,7 @@ struct Grid {
     int nev;           // events in the batch (mf_create_batch; 1 otherwise): blockIdx.y of every staged kernel is the event, whose cells
                        // sit at offset event*ncell (interior layout) / event*next (extended layout) inside each component array
     FastDiv dv[2][3];  // dv[a][m]: division by n[a] + m, a = x, y, m = 0, 1, 2: every row length an index space of this grid has
+    int cslot;         // first of this context's nev slots in the constant-memory copy of the step scalars, or -1: read them from StepState
 };
 
 // Per-step scalars that live in device memory so that a step never needs the host (A10).
@@ -54,6 +55,25 @@ struct StepState {
     int pad;
     long long steps;
 };
+
+// The scalars of a step that the hot kernels multiply with, also kept in CONSTANT memory (mf_stepconst.cuh): a constant-bank or
+// uniform-register operand is not read from the register file, and a DFMA with three distinct REGISTER operands occupies the FP64 pipe
+// for 3 cycles instead of 2 on B200 (measured: mf_probe_fp64, profiles/).  Negated forms are stored so that no operand needs a sign flip.
+struct StepConst {
+    double dt, lam, hl, c_lw, c_lf;     // as in StepState
+    double nc_lw;                       // -c_lw          (Eq.10 on the mean/half-jump form)
+    double nc2_lf;                      // -2 c_lf        (Eq.11)
+    double nhlam;                       // -lam/2         (Eq.8)
+};
+constexpr int MF_CSLOTS = 512;          // events (of all live contexts together) whose step scalars fit the constant bank: 32 KB
+
+// stage coefficients straight from the StepState in global memory (kernels without a constant-memory variant)
+__device__ __forceinline__ MustaCoef musta_coef_of(const StepState* ds)
+{
+    MustaCoef m;
+    m.lam = ds->lam; m.c_lw = ds->c_lw; m.c_lf = ds->c_lf; m.nc_lw = -m.c_lw; m.nc2_lf = -2.0 * m.c_lf; m.nhlam = -0.5 * m.lam;
+    return m;
+}
 
 struct Source {
     double dEdx, norm, inv_two_s2, x0, y0, z0;   // S = dEdx*norm*exp(-r^2*inv_two_s2)
