@@ -159,6 +159,20 @@ int mf_profile_read(mf_ctx*, double ms[MF_NCLASS], long long launches[MF_NCLASS]
  * out = { dfma/s with two register operands (x*a+a), dadd/s, dmul/s, rcp results/s, sqrt results/s, SM clock estimate in Hz, SM count,
  *         dfma/s with three distinct register operands (x = y*z + x; the register file delivers them in 3 cycles instead of 2) }. */
 int mf_probe_fp64(double out[8]);
+/* Conserved totals WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid it): out5[q] = scale * sum over ncells cells of (E, Mx, My, Mz, R)[q] (Eq.1's conserved quantities, :41-49; pass
+ * scale = dx^D for mf_conserved_totals' convention).  The five inputs and out5 (5 doubles) are DEVICE pointers owned by the caller; no
+ * context is needed.  The per-block partial sums that mf_conserved_totals keeps in a cudaMalloc'ed buffer live in a file-scope
+ * __device__ array of 40 KB that every GPU that loads the library holds until exit; ncells <= MF_STATIC_MAX_CELLS (2^24 = 256^3),
+ * larger sizes return MF_EINVAL (mf_static_last_error() says why).  Two kernel launches on cuda_stream (a cudaStream_t as void*, NULL =
+ * the default stream), asynchronous, no cudaMalloc/cudaFree, deterministic summation order.  Every call shares the array, which keeps
+ * the last call's contents (a call overwrites every slot it reads, so nothing has to be cleared): calls that OVERLAP on the GPU -
+ * different streams, several host threads on one device - race on it; serialise them. */
+#define MF_STATIC_MAX_CELLS (1LL << 24)
+int mf_totals_static(const double* E, const double* Mx, const double* My, const double* Mz, const double* R, long long ncells, double scale,
+                     double* out5, void* cuda_stream);
+const char* mf_static_last_error(void);     /* message of the calling thread's last failed mf_totals_static */
+
 /* Library build info: "mustaforce <version> sm_100a [strict]" */
 const char* mf_version(void);
 

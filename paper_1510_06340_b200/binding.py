@@ -62,6 +62,8 @@ SIGNATURES = {
     "mf_profile": (C.c_int, [_vp, C.c_int]),
     "mf_profile_read": (C.c_int, [_vp, _dp, C.POINTER(C.c_longlong)]),
     "mf_probe_fp64": (C.c_int, [_dp]),
+    "mf_totals_static": (C.c_int, [C.c_void_p] * 5 + [C.c_longlong, C.c_double, C.c_void_p, C.c_void_p]),
+    "mf_static_last_error": (C.c_char_p, []),
     "mf_version": (C.c_char_p, []),
 }
 
@@ -106,6 +108,17 @@ def probe_fp64(strict=False):
         raise MustaForceError(rc, "mf_probe_fp64 failed (no GPU?)")
     return dict(dfma_per_s=out[0], dadd_per_s=out[1], dmul_per_s=out[2], rcp_per_s=out[3], sqrt_per_s=out[4],
                 sm_clock_hz=out[5], sms=int(out[6]), dfma3_per_s=out[7])
+
+
+def totals_static(device_ptrs, ncells, scale, out_ptr, stream=None, strict=False):
+    """mf_totals_static: allocation-free conserved totals of five DEVICE arrays (integers such as torch's data_ptr()) into the device
+    array out_ptr (5 doubles), on `stream` (a cudaStream_t as int, None = default stream).  Argument marshalling only."""
+    lib = load(strict)
+    rc = lib.mf_totals_static(*[C.c_void_p(int(p)) for p in device_ptrs], int(ncells), float(scale), C.c_void_p(int(out_ptr)),
+                              C.c_void_p(int(stream)) if stream else None)
+    if rc != MF_OK:
+        raise MustaForceError(rc, lib.mf_static_last_error().decode())
+    return rc
 
 
 def version(strict=False):
