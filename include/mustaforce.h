@@ -123,6 +123,15 @@ int mf_get_path(mf_ctx*, int* path);        /* the path mf_step will actually ta
  * the results are bit-identical to the three-register form.  Frees (on = 1) or re-allocates (on = 0) the third register; synchronises.
  * Staged path only (MF_PATH_AUTO then resolves to it); MF_EINVAL if another path is selected. */
 int mf_set_low_storage(mf_ctx*, int on);
+/* Single-precision STATE ("The state of the system is saved as 5 single precision floating-point numbers
+ * per lattice cell"; reading A19): bits = 32 makes every STORED state value a float - the state handed in and the result of every Runge-Kutta
+ * stage are rounded to nearest even on the store - while all arithmetic between a load and the next store, the scratch (face states, fluxes)
+ * and the CFL reduction (taken from the stored, rounded U^n) stay fp64.  Halves the bytes of the state registers that cross HBM.  The calls
+ * that hand states in or out keep their double arrays (values are rounded on the way in and widened on the way out).  bits = 64 (default)
+ * restores the fp64 state.  The current state is converted; synchronises.  Staged path only (MF_PATH_AUTO then resolves to it); MF_EINVAL for
+ * another bit count or if another path is selected.  Outside BASELINE.json's fp64 contract: bench.py reports it beside the headline, never as it. */
+int mf_set_state_precision(mf_ctx*, int bits);
+int mf_get_state_precision(mf_ctx*, int* bits);
 /* mf_step / mf_step_dt replay whole steps from a CUDA graph when n >= 7 (5 in low-storage mode): one eager step, then one captured period of
  * the register rotation (3 steps, or 2) launched repeatedly, the remainder eagerly.  The launches and their arguments are exactly the eager
  * ones (every per-step scalar lives in device memory), so results are bit-identical; it removes the per-launch host cost that dominates

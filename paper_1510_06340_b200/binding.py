@@ -51,6 +51,8 @@ SIGNATURES = {
     "mf_set_path": (C.c_int, [_vp, C.c_int]),
     "mf_get_path": (C.c_int, [_vp, C.POINTER(C.c_int)]),
     "mf_set_low_storage": (C.c_int, [_vp, C.c_int]),
+    "mf_set_state_precision": (C.c_int, [_vp, C.c_int]),
+    "mf_get_state_precision": (C.c_int, [_vp, C.POINTER(C.c_int)]),
     "mf_set_graph": (C.c_int, [_vp, C.c_int]),
     "mf_graph_stats": (C.c_int, [_vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]),
     "mf_memory_bytes": (C.c_int, [_vp, C.POINTER(C.c_longlong)]),
@@ -130,7 +132,7 @@ class MustaForce:
     events stepped by the same launches, each on its own clock) every array has shape (B, nz, ny, nx)."""
 
     def __init__(self, nx, ny=1, nz=1, dx=1.0, limiter="minmod", k_stages=2, rk=2, bc="outflow", predictor=True,
-                 alpha=None, cs2=None, path="auto", stream=None, strict=False, eos_table=None, batch=None):
+                 alpha=None, cs2=None, path="auto", stream=None, strict=False, eos_table=None, batch=None, state_bits=64):
         self.lib = load(strict)
         self.batch = batch
         self.shape = (nz, ny, nx) if batch is None else (int(batch), nz, ny, nx)
@@ -155,6 +157,8 @@ class MustaForce:
             self.set_stream(stream)
         if eos_table is not None:
             self.set_eos_table(eos_table)
+        if state_bits != 64:
+            self.set_state_precision(state_bits)
 
     def _chk(self, rc, allow=()):
         if rc != MF_OK and rc not in allow:
@@ -251,6 +255,14 @@ class MustaForce:
 
     def set_low_storage(self, on):
         self._chk(self.lib.mf_set_low_storage(self.h, 1 if on else 0))
+
+    def set_state_precision(self, bits):
+        self._chk(self.lib.mf_set_state_precision(self.h, int(bits)))
+
+    def state_precision(self):
+        b = C.c_int()
+        self._chk(self.lib.mf_get_state_precision(self.h, C.byref(b)))
+        return b.value
 
     def set_graph(self, on):
         self._chk(self.lib.mf_set_graph(self.h, 1 if on else 0))

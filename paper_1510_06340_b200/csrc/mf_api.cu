@@ -103,6 +103,22 @@ int cuda_fail(mf_ctx* c, cudaError_t e, const char* what)
 CState5 cstate(const double* base, long long n) { CState5 s; for (int v = 0; v < 5; ++v) s.q[v] = base + v * n; return s; }
 State5 state(double* base, long long n) { State5 s; for (int v = 0; v < 5; ++v) s.q[v] = base + v * n; return s; }
 
+// Component pointers of a STATE REGISTER: nst elements per component of the context's state element type (double, or float in 32-bit state
+// mode, reading A19).  The structs carry double pointers either way; the kernels of the staged path cast them back (ld_state / st_state).
+CState5 creg(const mf_ctx* c, const double* base, long long first = 0)
+{
+    CState5 s;
+    for (int v = 0; v < 5; ++v)
+        s.q[v] = c->g.state32 ? reinterpret_cast<const double*>(reinterpret_cast<const float*>(base) + v * c->nst + first) : base + v * c->nst + first;
+    return s;
+}
+State5 reg(const mf_ctx* c, double* base)
+{
+    State5 s;
+    for (int v = 0; v < 5; ++v) s.q[v] = c->g.state32 ? reinterpret_cast<double*>(reinterpret_cast<float*>(base) + v * c->nst) : base + v * c->nst;
+    return s;
+}
+
 Faces faces_of(mf_ctx* c)
 {
     Faces f; memset(&f, 0, sizeof(f));
@@ -145,6 +161,12 @@ void clear_table(Eos& q)
 
 int resolve_path(mf_ctx* c)
 {
+    if (c->g.state32) {
+        // single-precision state: the kernels of the staged path carry the state element type (the sweep and tile kernels read doubles)
+        if (c->path_req != MF_PATH_AUTO && c->path_req != MF_PATH_STAGED) return MF_EINVAL;
+        c->path = MF_PATH_STAGED;
+        return MF_OK;
+    }
     if (c->nreg == 2) {
         // low storage: an RK stage writes its result over the register it read, which only the staged path's last kernel allows (it touches
         // the state at the thread's own cell only; the sweep and tile kernels read neighbours of the state they are replacing)
@@ -272,8 +294,11 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
         if (rc != MF_OK) return rc;
         Faces fc = faces_of(c);
         Fluxes fx = fluxes_of(c);
+        // state registers in the context's state element type (reading A19); the result of form 3 (mf_eval_L) is L itself, always double
+        const CState5 Vs = creg(c, V), Uas = creg(c, Ua);
+        const State5 outs = sg.form == 3 ? state(out, n) : reg(c, out);
         int ps = prof_begin(c, 1);
-        c->launches += launch_cell_stage(c->g, c->q, c->limiter, c->predictor, cstate(V, n), fc, c->ds, c->stream);
+        c->launches += launch_cell_stage(c->g, c->q, c->limiter, c->predictor, Vs, fc, c->ds, c->stream);
         prof_end(c, ps);
         if (c->g.act[0]) {
             // y and z fluxes to HBM, then the x fluxes fused with divergence + source + RK combine (F_x stays on chip)
@@ -281,14 +306,14 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
             c->launches += launch_flux_stage(c->g, c->q, c->k, 6, fc, fx, c->ds, c->stream);
             prof_end(c, ps);
             ps = prof_begin(c, 3);
-            c->launches += launch_xflux_combine(c->g, c->q, c->k, fc, fx, sg, cstate(Ua, n), cstate(V, n), state(out, n), c->src, c->ds, c->stream);
+            c->launches += launch_xflux_combine(c->g, c->q, c->k, fc, fx, sg, Uas, Vs, outs, c->src, c->ds, c->stream);
             prof_end(c, ps);
         } else {
             ps = prof_begin(c, 2);
             c->launches += launch_flux_stage(c->g, c->q, c->k, 7, fc, fx, c->ds, c->stream);
             prof_end(c, ps);
             ps = prof_begin(c, 3);
-            c->launches += launch_combine(c->g, c->q, fx, sg, cstate(Ua, n), cstate(V, n), state(out, n), c->src, c->ds, c->stream);
+            c->launches += launch_combine(c->g, c->q, fx, sg, Uas, Vs, outs, c->src, c->ds, c->stream);
             prof_end(c, ps);
         }
     }
@@ -553,6 +578,8 @@ int reset_after_set(mf_ctx* c)
     return check_launch(c);
 }
 
+// The caller's doubles land in register 0 as doubles (every register is allocated for doubles).  In 32-bit state mode finish_copy_in then
+// rounds them into register 1 as floats, which becomes U^n (reading A19: the state handed in is rounded once).
 int copy_in(mf_ctx* c, const double* const src[5], cudaMemcpyKind kind)
 {
     c->cur = 0;
@@ -561,11 +588,29 @@ int copy_in(mf_ctx* c, const double* const src[5], cudaMemcpyKind kind)
     return MF_OK;
 }
 
+int finish_copy_in(mf_ctx* c)
+{
+    if (!c->g.state32) return MF_OK;
+    c->launches += launch_state_convert(c->nst, 1, cstate(c->U[0], c->nst), reg(c, c->U[1]), c->num_sms, c->stream);
+    c->cur = 1;
+    return MF_OK;
+}
+
+// `base` holds doubles, nst per component
 int copy_out(mf_ctx* c, const double* base, double* const dst[5], cudaMemcpyKind kind)
 {
     for (int v = 0; v < 5; ++v)
         MF_CUDA(c, cudaMemcpyAsync(dst[v], base + v * c->nst, sizeof(double) * c->nst, kind, c->stream));
     return MF_OK;
+}
+
+// U^n as doubles: the register itself, or in 32-bit state mode its widened copy in the next (free between steps) register
+const double* state_as_doubles(mf_ctx* c)
+{
+    if (!c->g.state32) return c->U[c->cur];
+    double* scratch = c->U[(c->cur + 1) % c->nreg];
+    c->launches += launch_state_convert(c->nst, 0, creg(c, c->U[c->cur]), state(scratch, c->nst), c->num_sms, c->stream);
+    return scratch;
 }
 
 } // namespace
@@ -579,6 +624,7 @@ int mf_set_state(mf_ctx* c, const double* E, const double* Mx, const double* My,
     const double* src[5] = { E, Mx, My, Mz, R };
     int rc = copy_in(c, src, cudaMemcpyHostToDevice);
     if (rc != MF_OK) return rc;
+    finish_copy_in(c);
     if ((rc = reset_after_set(c)) != MF_OK) return rc;
     MF_CUDA(c, cudaStreamSynchronize(c->stream));
     return MF_OK;
@@ -591,6 +637,7 @@ int mf_set_state_device(mf_ctx* c, const double* E, const double* Mx, const doub
     const double* src[5] = { E, Mx, My, Mz, R };
     int rc = copy_in(c, src, cudaMemcpyDeviceToDevice);
     if (rc != MF_OK) return rc;
+    finish_copy_in(c);
     return reset_after_set(c);
 }
 
@@ -599,7 +646,7 @@ int mf_get_state(mf_ctx* c, double* E, double* Mx, double* My, double* Mz, doubl
     if (!c) return MF_EINVAL;
     if (!E || !Mx || !My || !Mz || !R) return fail(c, MF_EINVAL, "null pointer");
     double* dst[5] = { E, Mx, My, Mz, R };
-    int rc = copy_out(c, c->U[c->cur], dst, cudaMemcpyDeviceToHost);
+    int rc = copy_out(c, state_as_doubles(c), dst, cudaMemcpyDeviceToHost);
     if (rc != MF_OK) return rc;
     return fetch_step_state(c);
 }
@@ -609,7 +656,7 @@ int mf_get_state_device(mf_ctx* c, double* E, double* Mx, double* My, double* Mz
     if (!c) return MF_EINVAL;
     if (!E || !Mx || !My || !Mz || !R) return fail(c, MF_EINVAL, "null pointer");
     double* dst[5] = { E, Mx, My, Mz, R };
-    int rc = copy_out(c, c->U[c->cur], dst, cudaMemcpyDeviceToDevice);
+    int rc = copy_out(c, state_as_doubles(c), dst, cudaMemcpyDeviceToDevice);
     if (rc != MF_OK) return rc;
     return fetch_step_state(c);
 }
@@ -622,6 +669,7 @@ int mf_set_state_prim(mf_ctx* c, const double* e, const double* vx, const double
     int rc = copy_in(c, src, cudaMemcpyHostToDevice);
     if (rc != MF_OK) return rc;
     c->launches += launch_prim2con(c->g, c->q, state(c->U[0], c->nst), c->stream);      // Eq.4 on the device
+    finish_copy_in(c);
     if ((rc = reset_after_set(c)) != MF_OK) return rc;
     MF_CUDA(c, cudaStreamSynchronize(c->stream));
     return MF_OK;
@@ -632,7 +680,7 @@ int mf_get_state_prim(mf_ctx* c, double* e, double* vx, double* vy, double* vz, 
     if (!c) return MF_EINVAL;
     if (!e || !vx || !vy || !vz || !n) return fail(c, MF_EINVAL, "null pointer");
     double* scratch = c->U[(c->cur + 1) % c->nreg];
-    c->launches += launch_con2prim(c->g, c->q, cstate(c->U[c->cur], c->nst), state(scratch, c->nst), c->stream);
+    c->launches += launch_con2prim(c->g, c->q, creg(c, c->U[c->cur]), state(scratch, c->nst), c->stream);
     int rc = check_launch(c);
     if (rc != MF_OK) return rc;
     double* dst[5] = { e, vx, vy, vz, n };
@@ -656,7 +704,7 @@ static int enqueue_step(mf_ctx* c, int mode, double value)
 {
     if (mode == 0 && !c->smax_valid) {                            // otherwise the previous step's last combine already reduced U^n
         int ps = prof_begin(c, 0);
-        c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->nst), c->ds, c->num_sms, c->stream);   // a2, from U^n
+        c->launches += launch_cfl(c->g, c->q, creg(c, c->U[c->cur]), c->ds, c->num_sms, c->stream);   // a2, from U^n
         prof_end(c, ps);
     }
     int rc = begin_step(c, mode, value);
@@ -779,9 +827,8 @@ int mf_eval_L(mf_ctx* c, double dt, double* L_E, double* L_Mx, double* L_My, dou
 static int totals_of(mf_ctx* c, int event, double out[5])
 {
     Grid g = c->g;
-    CState5 U = cstate(c->U[c->cur], c->nst);
+    const CState5 U = creg(c, c->U[c->cur], event < 0 ? 0 : (long long)event * g.ncell);
     if (event < 0) g.ncell = c->nst;
-    else for (int v = 0; v < 5; ++v) U.q[v] += (long long)event * g.ncell;
     c->launches += launch_totals(g, U, c->partials, c->nblocks_tot, c->stream);
     int rc = check_launch(c);
     if (rc != MF_OK) return rc;
@@ -828,7 +875,7 @@ int mf_get_time(mf_ctx* c, double* t, double* last_dt, long long* steps) { retur
 int mf_max_signal_speed(mf_ctx* c, double* smax)
 {
     if (!c || !smax) return MF_EINVAL;
-    c->launches += launch_cfl(c->g, c->q, cstate(c->U[c->cur], c->nst), c->ds, c->num_sms, c->stream);
+    c->launches += launch_cfl(c->g, c->q, creg(c, c->U[c->cur]), c->ds, c->num_sms, c->stream);
     int rc = check_launch(c);
     if (rc != MF_OK) return rc;
     rc = fetch_step_state(c);
@@ -949,6 +996,36 @@ int mf_set_low_storage(mf_ctx* c, int on)
     }
     return MF_OK;
 }
+
+int mf_set_state_precision(mf_ctx* c, int bits)
+{
+    if (!c) return MF_EINVAL;
+    if (bits != 32 && bits != 64) return fail(c, MF_EINVAL, "state precision must be 32 or 64 bits");
+    const int on = bits == 32;
+    if (on == c->g.state32) return MF_OK;
+    c->epoch++;
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    const int keep = c->g.state32;
+    c->g.state32 = on;
+    if (resolve_path(c) != MF_OK) {
+        c->g.state32 = keep; resolve_path(c);
+        return fail(c, MF_EINVAL, "the single-precision state runs on the staged path only: select MF_PATH_AUTO or MF_PATH_STAGED first");
+    }
+    // the stored state changes its element type: U^n is converted into the next register (free between steps), which becomes U^n
+    const int next = (c->cur + 1) % c->nreg;
+    c->g.state32 = keep;                                           // creg / reg describe the source in its present type ...
+    const CState5 src = creg(c, c->U[c->cur]);
+    c->g.state32 = on;                                             // ... and the destination in the new one
+    c->launches += launch_state_convert(c->nst, on, src, reg(c, c->U[next]), c->num_sms, c->stream);
+    c->cur = next;
+    c->smax_valid = 0;                                             // S_max is taken from the stored (rounded) state
+    int rc = check_launch(c);
+    if (rc != MF_OK) return rc;
+    MF_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MF_OK;
+}
+
+int mf_get_state_precision(mf_ctx* c, int* bits) { if (!c || !bits) return MF_EINVAL; *bits = c->g.state32 ? 32 : 64; return MF_OK; }
 
 int mf_memory_bytes(mf_ctx* c, long long* bytes)
 {

@@ -567,6 +567,16 @@ __device__ __forceinline__ double signal_speed(const Eos& q, double E, double Mx
     return (av + cs) / (1.0 + av * cs);
 }
 
+// ---- reading A19 ("saved as 5 single precision floating-point numbers per lattice cell"): the state registers hold elements
+// of type ST (double, or float in 32-bit state mode).  The structs carry double pointers whatever ST is (the host computes them with the
+// element size of the mode); a load widens to double, a store rounds to nearest even, and every operation in between is fp64.
+template <class ST>
+__device__ __forceinline__ double ld_state(const double* base, unsigned int o) { return (double)reinterpret_cast<const ST*>(base)[o]; }
+template <class ST>
+__device__ __forceinline__ void st_state(double* base, unsigned int o, double x) { reinterpret_cast<ST*>(base)[o] = (ST)x; }
+template <class ST>
+__device__ __forceinline__ double as_stored(double x) { return (double)(ST)x; }      // the value a later load of the stored element returns
+
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
 // idx -> (a, b, c) with idx = a + d0*(b + d1*c), idx < 2^32 (mf_create refuses larger grids), by two multiply-shift divisions.

@@ -35,7 +35,7 @@ static inline unsigned int blocks_for(long long n, int tpb) { return (unsigned i
 
 
 // =========================================================================== a2: CFL reduction
-template <int EK>
+template <int EK, class ST>
 __global__ void __launch_bounds__(TPB) k_cfl(Grid g, Eos q, CState5 U, StepState* ds)
 {
     double smax = 0.0;
@@ -44,7 +44,8 @@ __global__ void __launch_bounds__(TPB) k_cfl(Grid g, Eos q, CState5 U, StepState
     const unsigned int stride = gridDim.x * blockDim.x;
     for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < (unsigned int)g.ncell; i += stride) {
         const unsigned int o = eo + i;
-        double s = signal_speed<EK>(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], U.q[4][o], bad);
+        double s = signal_speed<EK>(q, ld_state<ST>(U.q[0], o), ld_state<ST>(U.q[1], o), ld_state<ST>(U.q[2], o), ld_state<ST>(U.q[3], o),
+                                    ld_state<ST>(U.q[4], o), bad);
         smax = fmax(smax, s);
     }
     block_reduce_smax(smax, bad, ds + blockIdx.y);
@@ -57,7 +58,8 @@ int launch_cfl(const Grid& g, const Eos& q, CState5 U, StepState* ds, int num_sm
     if (cap < 1u) cap = 1u;
     if (nb > cap) nb = cap;
     const dim3 grid(nb, g.nev);
-    if (q.kind) k_cfl<1><<<grid, TPB, 0, st>>>(g, q, U, ds); else k_cfl<0><<<grid, TPB, 0, st>>>(g, q, U, ds);
+    if (g.state32) { if (q.kind) k_cfl<1, float><<<grid, TPB, 0, st>>>(g, q, U, ds); else k_cfl<0, float><<<grid, TPB, 0, st>>>(g, q, U, ds); }
+    else { if (q.kind) k_cfl<1, double><<<grid, TPB, 0, st>>>(g, q, U, ds); else k_cfl<0, double><<<grid, TPB, 0, st>>>(g, q, U, ds); }
     return 1;
 }
 
@@ -117,7 +119,7 @@ int launch_reset(StepState* ds, int nev, cudaStream_t st) { k_reset<<<(nev + 63)
 
 // =========================================================================== a3 + a4: cell stage
 // One thread per cell of the extended region (interior + 1 layer on every active axis).
-template <int LIM, int EK, bool UC>
+template <int LIM, int EK, bool UC, class ST>
 __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, int predictor, CState5 V, Faces fc, State5 Wout, const StepState* ds)
 {
     // linear index over the extended region, x fastest: 256 consecutive cells per block (measured on B200: 32 x 8 tiles, which
@@ -137,7 +139,7 @@ __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, 
     const unsigned int pu = blockIdx.y * (unsigned int)g.next + (unsigned int)p;
     double U0[5];
 #pragma unroll
-    for (int v = 0; v < 5; ++v) U0[v] = V.q[v][o0];
+    for (int v = 0; v < 5; ++v) U0[v] = ld_state<ST>(V.q[v], o0);
 #if MF_CELL_PF
     // The kernel is latency bound, and the only lines a block meets for the first time are those of the plane above (z+1): everything else
     // was touched by the blocks before it.  Pull that plane's lines for the cells one wave of blocks ahead towards L2.
@@ -145,7 +147,7 @@ __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, 
         const unsigned int opf = o0 + ns[2] + (unsigned int)MF_CELL_PF;
         if (opf < (blockIdx.y + 1u) * (unsigned int)g.ncell) {
 #pragma unroll
-            for (int v = 0; v < 5; ++v) prefetch_l2(&V.q[v][opf]);
+            for (int v = 0; v < 5; ++v) prefetch_l2(reinterpret_cast<const ST*>(V.q[v]) + opf);
         }
     }
 #endif
@@ -159,8 +161,8 @@ __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, 
         const unsigned int op = o0 + (unsigned int)(bc_index(c[d] + 1, g.n[d], g.periodic) - cc[d]) * ns[d];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
-            double a = U0[v] - V.q[v][om];
-            double b = V.q[v][op] - U0[v];
+            double a = U0[v] - ld_state<ST>(V.q[v], om);
+            double b = ld_state<ST>(V.q[v], op) - U0[v];
             double s = slope2<LIM>(a, b);                                  // Eq.15-17
             UL[d][v] = U0[v] - 0.5 * s;                                    // Eq.12 :161
             UR[d][v] = U0[v] + 0.5 * s;
@@ -214,7 +216,9 @@ __global__ void __launch_bounds__(CT, MF_CELL_MINB) k_cell_stage(Grid g, Eos q, 
             const unsigned int om = o0 + (unsigned int)(bc_index(c[d] - 1, g.n[d], g.periodic) - cc[d]) * ns[d];
             const unsigned int op = o0 + (unsigned int)(bc_index(c[d] + 1, g.n[d], g.periodic) - cc[d]) * ns[d];
 #pragma unroll
-            for (int v = 0; v < 5; ++v) { Um[d][v] = __ldg(&V.q[v][om]); Up[d][v] = __ldg(&V.q[v][op]); }
+            for (int v = 0; v < 5; ++v) {
+                Um[d][v] = (double)__ldg(reinterpret_cast<const ST*>(V.q[v]) + om); Up[d][v] = (double)__ldg(reinterpret_cast<const ST*>(V.q[v]) + op);
+            }
         }
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
@@ -270,11 +274,13 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
     State5 Wout;
     for (int v = 0; v < 5; ++v) Wout.q[v] = fc.f[g.act[0] ? 0 : (g.act[1] ? 1 : 2)][1][v];
     switch (limiter) {
-#define MF_CASE(L) case L: if (q.kind) k_cell_stage<L, 1, false><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); \
-                           else if (g.cslot >= 0) k_cell_stage<L, 0, true><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); \
-                           else k_cell_stage<L, 0, false><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); break;
+#define MF_CASE_ST(L, ST_) if (q.kind) k_cell_stage<L, 1, false, ST_><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); \
+                           else if (g.cslot >= 0) k_cell_stage<L, 0, true, ST_><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds); \
+                           else k_cell_stage<L, 0, false, ST_><<<nb, CT, 0, st>>>(g, q, predictor, V, fc, Wout, ds);
+#define MF_CASE(L) case L: if (g.state32) { MF_CASE_ST(L, float) } else { MF_CASE_ST(L, double) } break;
         MF_CASE(LIM_NONE) MF_CASE(LIM_MINMOD) MF_CASE(LIM_SUPERBEE) MF_CASE(LIM_VANALBADA) MF_CASE(LIM_VANLEER) MF_CASE(LIM_MC) MF_CASE(LIM_FIRST)
 #undef MF_CASE
+#undef MF_CASE_ST
     default: return 0;
     }
     return 1;
@@ -334,7 +340,7 @@ int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, F
 }
 
 // =========================================================================== a7 + a8: divergence, source, RK combine
-template <int EK>
+template <int EK, class ST>
 __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds)
 {
     const long long ol = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -358,8 +364,8 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
                 if (!g.act[d]) continue;
                 fhi[d][v] = fx.f[d][v][p]; flo[d][v] = fx.f[d][v][p - (unsigned int)g.es[d]];
             }
-            ua5[v] = sg.form == 3 ? 0.0 : Ua.q[v][o];
-            ub5[v] = (sg.form == 1 || sg.form == 2) ? Ub.q[v][o] : 0.0;
+            ua5[v] = sg.form == 3 ? 0.0 : ld_state<ST>(Ua.q[v], o);
+            ub5[v] = (sg.form == 1 || sg.form == 2) ? ld_state<ST>(Ub.q[v], o) : 0.0;
         }
         double W[5];
 #pragma unroll
@@ -380,7 +386,8 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
 #endif
             if (src.on && v < 2) L = L + S;
             W[v] = rk_form(sg, ua5[v], ub5[v], dt, L);
-            out.q[v][o] = W[v];
+            if (sg.form == 3) out.q[v][o] = W[v];                      // L itself (mf_eval_L): double whatever the state precision
+            else { st_state<ST>(out.q[v], o, W[v]); W[v] = as_stored<ST>(W[v]); }
         }
         if (sg.cfl) smax = signal_speed<EK>(q, W[0], W[1], W[2], W[3], W[4], bad);   // a2 for the next step, while U^{n+1} is in registers
     }
@@ -390,8 +397,13 @@ __global__ void __launch_bounds__(TPB) k_combine(Grid g, Eos q, Fluxes fx, Stage
 int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out, Source src, StepState* ds, cudaStream_t st)
 {
     const dim3 nb(blocks_for(g.ncell, TPB), g.nev);
-    if (q.kind) k_combine<1><<<nb, TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
-    else k_combine<0><<<nb, TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+    if (g.state32) {
+        if (q.kind) k_combine<1, float><<<nb, TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+        else k_combine<0, float><<<nb, TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+    } else {
+        if (q.kind) k_combine<1, double><<<nb, TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+        else k_combine<0, double><<<nb, TPB, 0, st>>>(g, q, fx, sg, Ua, Ub, out, src, ds);
+    }
     return 1;
 }
 
@@ -406,7 +418,7 @@ int launch_combine(const Grid& g, const Eos& q, Fluxes fx, Stage sg, CState5 Ua,
 // instead was 40% slower (the 35 KB per block cost the L1 hits of the x-neighbour loads).  History of this kernel: 1.56 -> 1.37 -> 1.03 -> 0.95 ms per launch.
 // FORM (the RK form of the stage) and CFL (last stage of a step) are compile-time: the stage loop has no form branches, and the
 // signal-speed code with its block reduction exists only in the instantiations that need it.
-template <int EK, int FORM, bool CFL, bool UC>
+template <int EK, int FORM, bool CFL, bool UC, class ST>
 __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q, int k, Faces fc, Fluxes fx, Stage sg, CState5 Ua, CState5 Ub, State5 out,
                                                           Source src, StepState* ds)
 {
@@ -447,8 +459,8 @@ __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q,
         for (int v = 0; v < 5; ++v) {
             if (g.act[1]) { fy1[v] = fx.f[1][v][pc]; fy0[v] = fx.f[1][v][pc - (unsigned int)g.es[1]]; }
             if (g.act[2]) { fz1[v] = fx.f[2][v][pc]; fz0[v] = fx.f[2][v][pc - (unsigned int)g.es[2]]; }
-            ua5[v] = FORM == 3 ? 0.0 : Ua.q[v][o];
-            ub5[v] = (FORM == 1 || FORM == 2) ? Ub.q[v][o] : 0.0;
+            ua5[v] = FORM == 3 ? 0.0 : ld_state<ST>(Ua.q[v], o);
+            ub5[v] = (FORM == 1 || FORM == 2) ? ld_state<ST>(Ub.q[v], o) : 0.0;
         }
     }
 #pragma unroll
@@ -474,9 +486,14 @@ __global__ void __launch_bounds__(XT, MF_XC_MINB) k_xflux_combine(Grid g, Eos q,
             if (src.on && v < 2) L = L + S;
             const double ua = ua5[v], ub = ub5[v];
             W[v] = FORM == 0 ? ua + dt * L : (FORM == 1 ? 0.5 * (ua + ub + dt * L) : (FORM == 2 ? sg.ca * ua + sg.cb * ub + (sg.cdt * dt) * L : L));
-            out.q[v][o] = W[v];
+            if (FORM == 3) out.q[v][o] = W[v];                             // L itself (mf_eval_L): double whatever the state precision
+            else st_state<ST>(out.q[v], o, W[v]);
         }
-        if (CFL) smax = signal_speed<EK>(q, W[0], W[1], W[2], W[3], W[4], bad);
+        if (CFL) {                                                         // S_max of the STORED (rounded, reading A19) new state
+#pragma unroll
+            for (int v = 0; v < 5; ++v) W[v] = as_stored<ST>(W[v]);
+            smax = signal_speed<EK>(q, W[0], W[1], W[2], W[3], W[4], bad);
+        }
     }
     if (CFL) block_reduce_smax<XT>(smax, bad, ds);
 }
@@ -486,8 +503,9 @@ int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx
 {
     const long long total = (long long)(g.n[0] + 1) * g.n[1] * g.n[2];
     const dim3 nb(blocks_for(total, XT - 1), g.nev);
-#define MF_XFC(EK_, FORM_, CFL_) do { if (EK_ == 0 && g.cslot >= 0) k_xflux_combine<EK_, FORM_, CFL_, EK_ == 0><<<nb, XT, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds); \
-                                      else k_xflux_combine<EK_, FORM_, CFL_, false><<<nb, XT, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds); } while (0)
+#define MF_XFC_ST(EK_, FORM_, CFL_, ST_) do { if (EK_ == 0 && g.cslot >= 0) k_xflux_combine<EK_, FORM_, CFL_, EK_ == 0, ST_><<<nb, XT, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds); \
+                                      else k_xflux_combine<EK_, FORM_, CFL_, false, ST_><<<nb, XT, 0, st>>>(g, q, k, fc, fx, sg, Ua, Ub, out, src, ds); } while (0)
+#define MF_XFC(EK_, FORM_, CFL_) do { if (g.state32) MF_XFC_ST(EK_, FORM_, CFL_, float); else MF_XFC_ST(EK_, FORM_, CFL_, double); } while (0)
 #define MF_XFC_FORMS(EK_) \
     if (sg.form == 0) { if (sg.cfl) MF_XFC(EK_, 0, true); else MF_XFC(EK_, 0, false); } \
     else if (sg.form == 1) { if (sg.cfl) MF_XFC(EK_, 1, true); else MF_XFC(EK_, 1, false); } \
@@ -496,6 +514,7 @@ int launch_xflux_combine(const Grid& g, const Eos& q, int k, Faces fc, Fluxes fx
     if (q.kind) { MF_XFC_FORMS(1) } else { MF_XFC_FORMS(0) }
 #undef MF_XFC_FORMS
 #undef MF_XFC
+#undef MF_XFC_ST
     return 1;
 }
 
@@ -513,16 +532,17 @@ __global__ void __launch_bounds__(TPB) k_prim2con(Grid g, Eos q, State5 U)
     U.q[0][o] = w - p; U.q[1][o] = w * vx; U.q[2][o] = w * vy; U.q[3][o] = w * vz; U.q[4][o] = n * sqrt(g2);
 }
 
-template <int EK>
+template <int EK, class ST>
 __global__ void __launch_bounds__(TPB) k_con2prim(Grid g, Eos q, CState5 U, State5 P)
 {
     const long long ol = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (ol >= g.ncell) return;
     const unsigned int o = blockIdx.y * (unsigned int)g.ncell + (unsigned int)ol;
     double vx, vy, vz, e, p;
-    velocity_pressure<EK>(q, U.q[0][o], U.q[1][o], U.q[2][o], U.q[3][o], U.q[4][o], vx, vy, vz, e, p);
+    const double R = ld_state<ST>(U.q[4], o);
+    velocity_pressure<EK>(q, ld_state<ST>(U.q[0], o), ld_state<ST>(U.q[1], o), ld_state<ST>(U.q[2], o), ld_state<ST>(U.q[3], o), R, vx, vy, vz, e, p);
     P.q[0][o] = e; P.q[1][o] = vx; P.q[2][o] = vy; P.q[3][o] = vz;
-    P.q[4][o] = U.q[4][o] * sqrt(1.0 - (vx * vx + vy * vy + vz * vz));   // n = R sqrt(1-v^2), Eq.23
+    P.q[4][o] = R * sqrt(1.0 - (vx * vx + vy * vy + vz * vz));           // n = R sqrt(1-v^2), Eq.23
 }
 
 int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st)
@@ -534,18 +554,20 @@ int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st)
 int launch_con2prim(const Grid& g, const Eos& q, CState5 U, State5 P, cudaStream_t st)
 {
     const dim3 nb(blocks_for(g.ncell, TPB), g.nev);
-    if (q.kind) k_con2prim<1><<<nb, TPB, 0, st>>>(g, q, U, P); else k_con2prim<0><<<nb, TPB, 0, st>>>(g, q, U, P);
+    if (g.state32) { if (q.kind) k_con2prim<1, float><<<nb, TPB, 0, st>>>(g, q, U, P); else k_con2prim<0, float><<<nb, TPB, 0, st>>>(g, q, U, P); }
+    else { if (q.kind) k_con2prim<1, double><<<nb, TPB, 0, st>>>(g, q, U, P); else k_con2prim<0, double><<<nb, TPB, 0, st>>>(g, q, U, P); }
     return 1;
 }
 
 // =========================================================================== totals: per-block partial sums (host adds them in long double)
+template <class ST>
 __global__ void __launch_bounds__(TPB) k_totals(Grid g, CState5 U, double* partials)
 {
     double acc[5] = { 0, 0, 0, 0, 0 };
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < g.ncell; o += stride)
 #pragma unroll
-        for (int v = 0; v < 5; ++v) acc[v] += U.q[v][o];
+        for (int v = 0; v < 5; ++v) acc[v] += (double)reinterpret_cast<const ST*>(U.q[v])[o];
     __shared__ double s[5][TPB / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
@@ -564,7 +586,31 @@ __global__ void __launch_bounds__(TPB) k_totals(Grid g, CState5 U, double* parti
 
 int launch_totals(const Grid& g, CState5 U, double* partials, int nblocks, cudaStream_t st)
 {
-    k_totals<<<nblocks, TPB, 0, st>>>(g, U, partials);
+    if (g.state32) k_totals<float><<<nblocks, TPB, 0, st>>>(g, U, partials); else k_totals<double><<<nblocks, TPB, 0, st>>>(g, U, partials);
+    return 1;
+}
+
+// =========================================================================== state precision (reading A19): double <-> float copies of a state
+// n elements per component; `src`/`dst` component pointers are already spaced for their own element type
+__global__ void __launch_bounds__(TPB) k_state_to_f32(long long n, CState5 src, State5 dst)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += stride)
+#pragma unroll
+        for (int v = 0; v < 5; ++v) reinterpret_cast<float*>(dst.q[v])[o] = (float)src.q[v][o];       // round to nearest even
+}
+__global__ void __launch_bounds__(TPB) k_state_to_f64(long long n, CState5 src, State5 dst)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += stride)
+#pragma unroll
+        for (int v = 0; v < 5; ++v) dst.q[v][o] = (double)reinterpret_cast<const float*>(src.q[v])[o];
+}
+int launch_state_convert(long long n, int to_f32, CState5 src, State5 dst, int num_sms, cudaStream_t st)
+{
+    long long nb = (n + TPB - 1) / TPB;
+    if (nb > 32LL * num_sms) nb = 32LL * num_sms;
+    if (to_f32) k_state_to_f32<<<(unsigned int)nb, TPB, 0, st>>>(n, src, dst); else k_state_to_f64<<<(unsigned int)nb, TPB, 0, st>>>(n, src, dst);
     return 1;
 }
 

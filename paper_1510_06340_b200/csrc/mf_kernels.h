@@ -62,6 +62,9 @@ int launch_sweep_xcombine(const Grid& g, const Eos& q, int limiter, int k, bool 
 int launch_prim2con(const Grid& g, const Eos& q, State5 U, cudaStream_t st);          // in place: (e,v,n) -> (E,M,R), Eq.4
 int launch_con2prim(const Grid& g, const Eos& q, CState5 U, State5 P, cudaStream_t st); // Eq.23
 int launch_totals(const Grid& g, CState5 U, double* partials /* 5*nblocks */, int nblocks, cudaStream_t st);
+// reading A19: copy a state of n elements per component from double to float (to_f32, round to nearest even) or from float to double;
+// the component pointers of src and dst are spaced for their own element type
+int launch_state_convert(long long n, int to_f32, CState5 src, State5 dst, int num_sms, cudaStream_t st);
 
 // ---- FP64 pipe micro-benchmarks (mf_probe_fp64; diagnostic, not on the hot path)
 int probe_fp64(double out[8]);

@@ -40,6 +40,7 @@ struct Grid {
                        // sit at offset event*ncell (interior layout) / event*next (extended layout) inside each component array
     FastDiv dv[2][3];  // dv[a][m]: division by n[a] + m, a = x, y, m = 0, 1, 2: every row length an index space of this grid has
     int cslot;         // first of this context's nev slots in the constant-memory copy of the step scalars, or -1: read them from StepState
+    int state32;       // 1: the state registers hold single-precision values (mf_set_state_precision, reading A19)
 };
 
 // Per-step scalars that live in device memory so that a step never needs the host (A10).
