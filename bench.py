@@ -33,39 +33,48 @@ UNIT = "cell-updates/s"
 
 # ----------------------------------------------------------------------------------------------------------------
 # Algorithmic work per cell-update.  FP64-pipe issue SLOTS:
-# add/sub/mul/fma/compare/min/max = 1, divide = 8, square root = 8 (a Newton sequence each); abs/neg/select = 0.
+# add/sub/mul/fma/compare/min/max = 1, abs/neg/select = 0, and two conventions for the divide and the square root:
+#   "survey"  (the frozen round-1 denominator): divide = 8, square root = 8, one flux evaluation 16 + 8 + 8 = 32;
+#   "minimal" (what the product code demonstrates, mf_device.cuh flux_fast: Newton reciprocal 3, Newton root 6, F_E = M_d): flux = 24.
+# The survey count is ABOVE the instructions the kernels issue (644 slots against ~485 FP64 instructions per MUSTA interface, k = 3), so
+# a fraction of it flatters the FP64 pipe; bench.py reports both, and the minimal one is the figure to compare with pipe utilisation.
 DIV, SQRT = 8, 8
 FLUX = 16 + DIV + SQRT                    # a6: one flux evaluation with con2prim             = 32
+DIV_MIN, SQRT_MIN, FLUX_MIN = 3, 6, 24
 SLOPE = {"none": 2, "first": 0, "minmod": 3, "superbee": 7, "mc": 8, "vanleer": 4 + DIV, "vanalbada": 6 + DIV}
+SLOPE_MIN = {"none": 2, "first": 0, "minmod": 3, "superbee": 7, "mc": 8, "vanleer": 4 + DIV_MIN, "vanalbada": 6 + DIV_MIN}
 
 
-def alg_slots(limiter, k, rk, ndim, predictor=True):
+def alg_slots(limiter, k, rk, ndim, predictor=True, minimal=False):
     """(slots per cell-update, slots per L-evaluation, slots of the MUSTA fluxes per L-evaluation)."""
-    recon = 5 * ndim * (4 + SLOPE[limiter])                        # a3: a, b, slope, two face values
-    pred = (2 * ndim * FLUX + 5 * 4 * ndim) if predictor else 0     # a4: 2D flux evaluations + delta + 2D face updates
-    force = 3 * FLUX + 50                                           # Eq.9-11: three fluxes + 10 per component
+    flux, div, sqrt, slope = (FLUX_MIN, DIV_MIN, SQRT_MIN, SLOPE_MIN) if minimal else (FLUX, DIV, SQRT, SLOPE)
+    recon = 5 * ndim * (4 + slope[limiter])                         # a3: a, b, slope, two face values
+    pred = (2 * ndim * flux + 5 * 4 * ndim) if predictor else 0     # a4: 2D flux evaluations + delta + 2D face updates
+    force = 3 * flux + 50                                           # Eq.9-11: three fluxes + 10 per component
     musta = (k + 1) * force + 20 * k                                # a5: k Eq.8 updates
     comb = 5 * (2 * ndim + 5)                                       # a7: divergence + RK form
-    cfl = (16 + DIV + SQRT) + (3 + SQRT) + (2 + DIV) + 1            # a2
+    cfl = (16 + div + sqrt) + (3 + sqrt) + (2 + div) + 1            # a2
     per_L = recon + pred + ndim * musta + comb
     return rk * per_L + cfl, per_L, ndim * musta
 
 
-def class_work(path, limiter, k, ndim, x_active, predictor=True):
+def class_work(path, limiter, k, ndim, x_active, predictor=True, state_bytes=8):
     """Algorithmic (FP64 slots, HBM bytes) per cell of one launch group of each kernel class, for one RK stage.
-    Bytes are what that kernel must read and write given the data layout of DESIGN.md section 4."""
+    Bytes are what that kernel must read and write given the data layout of DESIGN.md section 4; `state_bytes` is the size of a stored
+    state element (8, or 4 in single-precision state mode, staged path only: the scratch stays fp64)."""
+    sb = 5 * state_bytes                                                       # one state, per cell
     recon = 5 * ndim * (4 + SLOPE[limiter])
     pred = (2 * ndim * FLUX + 5 * 4 * ndim) if predictor else 0
     musta = (k + 1) * (3 * FLUX + 50) + 20 * k
     comb = 5 * (2 * ndim + 5)
     if path == "staged":
         nflux = ndim - 1 if x_active else ndim
-        out = {"cell_stage": (recon + pred, 40 + 40 * (1 + ndim)),            # U in; W and the half slopes H_d out
+        out = {"cell_stage": (recon + pred, sb + 40 * (1 + ndim)),            # U in; W and the half slopes H_d out
                "flux_stage": (nflux * musta, nflux * 120)}                    # W, H_d in, F_d out, per direction
         if x_active:
-            out["combine"] = (musta + comb, 80 + 40 * (ndim - 1) + 80 + 40)   # W, H_x, F_y, F_z, U^n, U_(s) in; new state out
+            out["combine"] = (musta + comb, 80 + 40 * (ndim - 1) + 2 * sb + sb)   # W, H_x, F_y, F_z, U^n, U_(s) in; new state out
         else:
-            out["combine"] = (comb, 40 * ndim + 80 + 40)
+            out["combine"] = (comb, 40 * ndim + 2 * sb + sb)
         return out
     if path == "sweep":
         # the sweep kernels limit their own slopes (one direction's share of the reconstruction each) from U; with the predictor on a
@@ -82,16 +91,20 @@ def class_work(path, limiter, k, ndim, x_active, predictor=True):
     return {"cell_stage": (recon + pred, 80), "fused_stage": (recon + ndim * musta + comb, 80 + 80 + 40)}   # fused: delta kernel + tile kernel
 
 
-def alg_bytes(rk):
-    """Minimum HBM bytes per cell-update: stage 1 reads U^n writes U1 (80 B), later stages read U_s and U^n, write (120 B); CFL +32 B."""
-    return 80 + 120 * (rk - 1) + 32
+def alg_bytes(rk, state_bytes=8):
+    """Minimum HBM bytes per cell-update: stage 1 reads U^n writes U1 (80 B), later stages read U_s and U^n, write (120 B); CFL +32 B
+    (halved with a single-precision state)."""
+    return (80 + 120 * (rk - 1) + 32) * state_bytes // 8
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch group at 256^3 (config 3 scheme), one ncu --set full capture per path:
-# staged: k_cell_stage 3.398 GB; k_flux_stage<1>, <2> 2.033 + 2.033 GB; k_xflux_combine 4.719 GB (profiles/r01_ncu_full_staged_256.md)
-# sweep (predictor off): k_sweep_flux<1>, <2> 1.325 + 1.340 GB; k_sweep_xcombine 3.359 GB (profiles/r01_ncu_full_sweep_256.md)
-NCU_TRAFFIC_GB_256 = {("staged", True): {"cell_stage": 3.398, "flux_stage": 4.066, "combine": 4.719},
-                      ("sweep", False): {"flux_stage": 2.664, "combine": 3.359}}
+# DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum per launch group, GB) of the kernels of THIS workload and path, from the ncu
+# --set full captures committed under profiles/ - measured once under ncu, not during this run: the JSON line names the file
+# ("traffic_source"), and nothing is reported for a workload, path or state precision without a committed capture.
+NCU_TRAFFIC_256 = {
+    ("staged", True): ("profiles/r02_ncu_full_staged_256.md", {"cell_stage": 3.398, "flux_stage": 4.066, "combine": 4.719}),
+    ("hybrid", True): ("profiles/r02_ncu_hybrid_tile3_256.md", {"fused_stage": 5.602}),
+    ("sweep", False): ("profiles/r01_ncu_full_sweep_256.md", {"flux_stage": 2.664, "combine": 3.359}),
+}
 
 FP64_LANES_PER_SM = 64       # B200 (sm_100): 4 SMSPs x 16 FP64 lanes; mf_probe_fp64 measures it (DESIGN.md)
 
@@ -279,7 +292,7 @@ def run_ours(args):
     with torch.cuda.stream(stream):
         eos_table = workloads.crossover_eos_table() if args.eos == "table" else None     # 8(f) row 1; not the metric's workload
         g = MustaForce(nx, ny, nz, dx=st["dx"], path=args.path, stream=stream.cuda_stream, eos_table=eos_table,
-                       batch=nbatch if nbatch > 1 else None, **sch)
+                       batch=nbatch if nbatch > 1 else None, state_bits=32 if args.state == "f32" else 64, **sch)
         if "jet" in st:
             j = st["jet"]
             g.set_jet_source(j["dEdx"], j["sigma"], j["x0"], j["y0"], j["z0"])
@@ -339,10 +352,12 @@ def run_ours(args):
 
     pk = peaks()
     pred_on = sch.get("predictor", True)
+    state_bytes = 4 if args.state == "f32" else 8
     slots_cu, slots_L, slots_musta = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim, pred_on)
+    slots_cu_min = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim, pred_on, minimal=True)[0]
     alu_peak_slots = 148 * FP64_LANES_PER_SM * pk["sm_max_mhz"] * 1e6          # FP64 instructions/s, all SMs
     # dominant kernel, from the event pairs recorded around every launch inside the timed region
-    work = class_work(g.path(), sch["limiter"], sch["k_stages"], ndim, nx > 1, pred_on)
+    work = class_work(g.path(), sch["limiter"], sch["k_stages"], ndim, nx > 1, pred_on, state_bytes)
     kernels = {}
     for name, (ms, groups) in prof.items():
         if name not in work or groups == 0:
@@ -357,11 +372,17 @@ def run_ours(args):
         kernels[name] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak, "traffic": None,
                          "kernel": name, "launch_ms": ms / groups, "share_of_step": ms / elapsed_ms,
                          "alg_slots_per_cell": slots, "alg_bytes_per_cell": nbytes}
-    # DRAM traffic per launch group from the committed ncu --set full capture of this same workload and path (profiles/r01_ncu_full_*_256.md)
-    if (nx, ny, nz) == (256, 256, 256) and sch["k_stages"] == 3 and sch["rk"] == 3 and nbatch == 1 and args.eos == "cs2":
-        for name, gb in NCU_TRAFFIC_GB_256.get((g.path(), bool(pred_on)), {}).items():
+    # DRAM traffic per launch group: only from a committed ncu --set full capture of this same workload, path and state precision
+    dram_step = None
+    if (nx, ny, nz) == (256, 256, 256) and sch["k_stages"] == 3 and sch["rk"] == 3 and nbatch == 1 and args.eos == "cs2" and \
+            state_bytes == 8 and (g.path(), bool(pred_on)) in NCU_TRAFFIC_256:
+        source, table = NCU_TRAFFIC_256[(g.path(), bool(pred_on))]
+        for name, gb in table.items():
             if name in kernels:
                 kernels[name]["traffic"] = gb * 1e9
+                kernels[name]["traffic_source"] = source + " (one ncu --set full capture of this workload and path; not measured in this run)"
+        if all(name in kernels or name == "cfl" for name in prof if prof[name][1]) and all(k_ in table for k_ in kernels):
+            dram_step = sch["rk"] * sum(table.values()) * 1e9
     # the dominant kernel class = the one with the largest share of the timed region
     roof = max(kernels.values(), key=lambda r: r["share_of_step"]) if kernels else None
     if roof:
@@ -369,7 +390,8 @@ def run_ours(args):
                                "lanes x clocks.max.sm; hbm: algorithmic bytes of that kernel / measured copy bandwidth; launch_ms is one "
                                "launch group (the class's launches of one RK stage) from CUDA-event pairs on the library's stream")
     step_frac_alu = (slots_cu * cells * args.steps / (elapsed_ms * 1e-3)) / alu_peak_slots
-    step_frac_hbm = (alg_bytes(sch["rk"]) * cells * args.steps / (elapsed_ms * 1e-3)) / (pk["hbm_gbs"] * 1e9)
+    step_frac_alu_min = (slots_cu_min * cells * args.steps / (elapsed_ms * 1e-3)) / alu_peak_slots
+    step_frac_hbm = (alg_bytes(sch["rk"], state_bytes) * cells * args.steps / (elapsed_ms * 1e-3)) / (pk["hbm_gbs"] * 1e9)
     probe = binding.probe_fp64()
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -377,6 +399,9 @@ def run_ours(args):
             "config": describe(st, {"path": g.path(), "l2": "state registers (%.0f MB each) exceed the 126 MB L2" % (40e-6 * cells)
                                     if 40 * cells > 126e6 else "state fits in L2 (small grid)", "parallelism": "replicas x%d" % world,
                                     "batch": "%d events per launch (mf_create_batch), each on its own dt" % nbatch if nbatch > 1 else "single event",
+                                    "state": "fp64 state registers" if state_bytes == 8 else
+                                    "single-precision STATE (PAPER.md:250, reading A19; arithmetic and scratch stay fp64) - outside "
+                                    "BASELINE.json's fp64 contract, reported beside the headline, never as it",
                                     "status": status, "eos": "p = e/3 (closed-form con2prim)" if args.eos == "cs2" else
                                     "tabulated crossover p(e,n), Newton con2prim (roofline fractions below use the closed-form slot count)"}),
             "clocks": clocks,
@@ -385,8 +410,14 @@ def run_ours(args):
             "gpu_launches": launches,
             "roofline": roof,
             "roofline_kernels": kernels,
-            "roofline_step": {"alg_slots_per_cell_update": slots_cu, "alg_bytes_per_cell_update": alg_bytes(sch["rk"]),
+            "roofline_step": {"alg_slots_per_cell_update": slots_cu, "alg_bytes_per_cell_update": alg_bytes(sch["rk"], state_bytes),
                               "frac_alu": step_frac_alu, "frac_hbm": step_frac_hbm, "hbm_peak": pk["hbm_source"],
+                              "alg_slots_minimal_per_cell_update": slots_cu_min, "frac_alu_minimal": step_frac_alu_min,
+                              "slots_note": "frac_alu counts divide = square root = 8 slots and 32 per flux evaluation (SURVEY.md 8(d), the "
+                                            "frozen denominator); frac_alu_minimal counts the sequences the product code issues (reciprocal 3, "
+                                            "root 6, flux 24) and is the figure to read as FP64-pipe utilisation of useful work",
+                              "dram_bytes_per_step": dram_step,
+                              "dram_over_alg_bytes": (dram_step / (alg_bytes(sch["rk"], state_bytes) * cells)) if dram_step else None,
                               "measured_dfma_per_s": probe["dfma_per_s"], "measured_rcp_slots": probe["dfma_per_s"] / probe["rcp_per_s"],
                               "measured_sqrt_slots": probe["dfma_per_s"] / probe["sqrt_per_s"]},
             "kernels_ms": {k: {"ms_total": v[0], "groups": v[1]} for k, v in prof.items()}}
@@ -407,6 +438,8 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid", "sweep"])
     ap.add_argument("--eos", default="cs2", choices=["cs2", "table"], help="table: synthetic crossover p(e,n) table with Newton con2prim")
     ap.add_argument("--predictor", default="on", choices=["on", "off"], help="off: without the Hancock half step (reading A4), reported beside the default")
+    ap.add_argument("--state", default="f64", choices=["f64", "f32"],
+                    help="f32: single-precision stored state (PAPER.md:250, reading A19), staged path; not the headline")
     ap.add_argument("--batch", type=int, default=1, help="events per context (mf_create_batch); config 4: the seeded events 0..B-1")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--ref-crop", type=int, default=64, help="edge of the centred crop the CPU oracle is timed on")

@@ -320,6 +320,12 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
     return MF_OK;
 }
 
+// does the last kernel of a step also reduce S_max of the new state (a2) for the next step's dt?
+bool last_stage_reduces_cfl(const mf_ctx* c)
+{
+    return c->path == MF_PATH_STAGED || c->path == MF_PATH_SWEEP || (c->path == MF_PATH_HYBRID && tile_reduces_cfl());
+}
+
 // RK2 (Eq.6 :103-105) / RK3 (Eq.7 :110-114); per-step scalars are already in c->ds.
 int run_step(mf_ctx* c)
 {
@@ -352,7 +358,7 @@ int run_step(mf_ctx* c)
     if (c->rk == 2) {
         Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
         Stage s2 = { 1, 0.5, 0.5, 1.0, 1.0 };
-        s2.cfl = c->path == MF_PATH_STAGED || c->path == MF_PATH_SWEEP;
+        s2.cfl = last_stage_reduces_cfl(c);
         if ((rc = run_stage(c, Un, s1, Un, Ra)) != MF_OK) return rc;
         if ((rc = run_stage(c, Ra, s2, Un, Rb)) != MF_OK) return rc;
         c->cur = (c->cur + 2) % 3;
@@ -360,14 +366,14 @@ int run_step(mf_ctx* c)
         Stage s1 = { 0, 1.0, 0.0, 1.0, 0.0 };
         Stage s2 = { 2, 0.75, 0.25, 0.25, 1.0 };
         Stage s3 = { 2, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, 0.5 };
-        s3.cfl = c->path == MF_PATH_STAGED || c->path == MF_PATH_SWEEP;
+        s3.cfl = last_stage_reduces_cfl(c);
         if ((rc = run_stage(c, Un, s1, Un, Ra)) != MF_OK) return rc;
         if ((rc = run_stage(c, Ra, s2, Un, Rb)) != MF_OK) return rc;
         if ((rc = run_stage(c, Rb, s3, Un, Ra)) != MF_OK) return rc;
         c->cur = (c->cur + 1) % 3;
     }
     c->launches += launch_end_step(c->ds, c->nev, c->stream);
-    c->smax_valid = c->path == MF_PATH_STAGED || c->path == MF_PATH_SWEEP;
+    c->smax_valid = last_stage_reduces_cfl(c);
     return MF_OK;
 }
 
@@ -694,6 +700,9 @@ static int begin_step(mf_ctx* c, int mode, double value)
     c->launches += launch_begin_step(c->ds, c->dsc, c->nev, mode, value, c->g.dx, c->alpha, c->stream);
     if (c->g.cslot >= 0 && (c->path == MF_PATH_STAGED || c->path == MF_PATH_HYBRID)) {
         if (upload_step_const_staged(c->dsc, c->g.cslot, c->nev, c->stream) != 0) { cudaGetLastError(); return fail(c, MF_ECUDA, "copy of the step scalars to constant memory failed"); }
+    }
+    if (c->g.cslot >= 0 && c->path == MF_PATH_HYBRID) {
+        if (upload_step_const_tile(c->dsc, c->g.cslot, c->nev, c->stream) != 0) { cudaGetLastError(); return fail(c, MF_ECUDA, "copy of the step scalars to constant memory failed"); }
     }
     return MF_OK;
 }

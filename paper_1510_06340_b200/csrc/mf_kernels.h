@@ -48,8 +48,12 @@ int launch_fused_stage(const Grid& g, const Eos& q, int limiter, int predictor, 
 int launch_tile_stage(const Grid& g, const Eos& q, int limiter, int predictor, int k, CState5 V, CState5 D, Stage sg, CState5 Ua, State5 out,
                       Source src, const StepState* ds, int num_sms, cudaStream_t st);
 
+// hybrid path: W and the half slopes from launch_cell_stage's scratch; all three flux directions, divergence, source, RK combine and (sg.cfl)
+// the CFL reduction of the new state in one kernel
 int launch_tile_stage_pre(const Grid& g, const Eos& q, int k, Faces fc, CState5 V, Stage sg, CState5 Ua, State5 out, Source src,
-                          const StepState* ds, int num_sms, cudaStream_t st);
+                          StepState* ds, int num_sms, cudaStream_t st);
+int upload_step_const_tile(const StepConst* dsc, int slot, int nev, cudaStream_t st);   // the tile unit's constant-memory step scalars; 0 = ok
+bool tile_reduces_cfl();
 
 // ---- sweep path (MF_PATH_SWEEP, mf_sweep.cu): per-direction sweeps that limit the slopes themselves from a +-2-cell halo of V; with pred the
 // Hancock increment Dl (extended layout, from launch_delta_stage) is added to both face states.  F_y, F_z go to fx, the x sweep finishes the cells.

@@ -13,6 +13,7 @@
 // Arithmetic per cell and per interface is the staged path's, in the same order: the strict build stays bit-identical to the oracle.
 #include "mf_kernels.h"
 #include "mf_blocks.cuh"
+#include "mf_stepconst.cuh"
 #include <cuda/barrier>
 #include <cstring>
 
@@ -254,6 +255,170 @@ k_tile_stage(Grid g, Eos q, int predictor, int k, int TZ, int ntx, int nty, CSta
 
 } // namespace
 
+// ================================================================================================ hybrid path, second form
+// k_tile3: the three flux directions + divergence + source + RK combine (+ CFL reduction) of one RK stage, fed by the cell stage's scratch
+// (W = U + delta and the half slopes H_d in the extended layout, so no boundary mapping here).  Same tile and z march as k_tile_stage, but
+//   * every interface task loads its own operands from global memory (L1/L2), exactly like the staged flux kernels do - there is no
+//     "cell part" phase, no face-state staging in shared memory and no barrier in front of the tasks;
+//   * only the finished fluxes go through shared memory (F_x, F_y double-buffered by plane parity, F_z in a thread-private slot), and the
+//     divergence of plane kk-1 is formed one iteration later, right after the z interface kk-1/2 that completes it;
+//   * ONE split barrier per plane: arrive after the x and y fluxes of plane kk are stored, wait after the next iteration's z MUSTA - a
+//     third of an iteration's work lies between the two, so the wait rarely blocks;
+//   * the lines of the next plane (W, H_x, H_y, H_z, U^n, U_(s)) are pulled towards L2 by one prefetch per 128 B line, not per thread;
+//   * the signal speed of the new state goes into the block reduction on the last stage (a2), so the hybrid path needs no separate CFL pass.
+// Iteration kk:  z task (kk-1/2) | wait(kk-1) | combine plane kk-1 | x tasks, y tasks of plane kk -> sF[kk&1] | arrive(kk)
+template <bool CFL, bool UC>
+__global__ void __launch_bounds__(NT, 3)
+k_tile3(Grid g, Eos q, int k, int TZ, int ntx, int nty, Faces fc, CState5 Wc, CState5 V, Stage sg, CState5 Ua, State5 out, Source src, StepState* ds)
+{
+    __shared__ double sFx[2][5][NFX];
+    __shared__ double sFy[2][5][NT];
+    __shared__ double sFz[5][TX * TY];
+#pragma nv_diag_suppress static_var_with_dynamic_init
+    __shared__ cuda::barrier<cuda::thread_scope_block> bar;
+#pragma nv_diag_default static_var_with_dynamic_init
+    if (threadIdx.x == 0) init(&bar, NT);
+    __syncthreads();
+
+    const int t = threadIdx.x;
+    const int item = blockIdx.x;
+    const int tx = item % ntx, ty = (item / ntx) % nty, tz = item / (ntx * nty);
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const int x0 = tx * TX, y0 = ty * TY;
+    const int z0 = tz * TZ, z1 = min(z0 + TZ, nz);
+    const StepConst sc = step_scalars<UC>(g, ds);
+    const MustaCoef mcf = musta_coef(sc);
+    const unsigned int es1 = (unsigned int)g.es[1], es2 = (unsigned int)g.es[2], ns1 = (unsigned int)g.ns[1], ns2 = (unsigned int)g.ns[2];
+
+    // ---- roles of this thread, fixed for the whole march.  Offsets are in-plane; the plane is added per iteration.
+    // x task: interface f = t % 33 of row j = t / 33, between cells (x0+f-1, y0+j) and (x0+f, y0+j); xp = extended offset of the left cell
+    const int xf = t % (TX + 1), xj = t / (TX + 1);
+    const bool xtask = t < NFX && x0 + xf <= nx && y0 + xj < ny;
+    const unsigned int xp = (unsigned int)(x0 + xf) + (unsigned int)(y0 + xj + 1) * es1;
+    // y task: interface f = t / 32 of column i = t % 32, between cells (x0+i, y0+f-1) and (x0+i, y0+f); yp = extended offset of the lower cell
+    const int yi = t % TX, yf = t / TX;
+    const bool ytask = x0 + yi < nx && y0 + yf <= ny;
+    const unsigned int yp = (unsigned int)(x0 + yi + 1) + (unsigned int)(y0 + yf) * es1;
+    // own cell (z task, combine): t = cj*32 + ci
+    const int ci = yi, cj = yf;
+    const int gx = x0 + ci, gy = y0 + cj;
+    const bool cell_ok = cj < TY && gx < nx && gy < ny;
+    const unsigned int co = (unsigned int)gx + (unsigned int)gy * ns1, cpe = (unsigned int)(gx + 1) + (unsigned int)(gy + 1) * es1;
+
+    double smax = 0.0;
+    int bad = 0;
+    cuda::barrier<cuda::thread_scope_block>::arrival_token token;
+    for (int kk = z0; kk <= z1; ++kk) {
+        const int buf = kk & 1;
+        // ---------------------------------------------------------------- lines of the next plane towards L2: one prefetch per line
+        if (kk + 1 < z1) {
+            if (t < 20 * (TY + 2)) {                                 // W, H_x, H_y, H_z (5 components each), rows y0-1 .. y0+TY of the tile
+                const int a = t / (TY + 2), r = t - a * (TY + 2);
+                if (y0 + r <= ny + 1) {
+                    // (no run-time index into the kernel parameters: the scratch arrays are consecutive slots of one allocation - H_x 0..4, W 5..9,
+                    //  H_y 10..14, H_z 20..24 in units of g.next, see faces_of in mf_api.cu)
+                    const double* base = fc.f[0][0][0] + (unsigned long long)(a < 15 ? a : a + 5) * (unsigned long long)g.next;
+                    const char* p0 = reinterpret_cast<const char*>(base + (unsigned int)x0 + (unsigned int)(y0 + r) * es1 + (unsigned int)(kk + 2) * es2);
+                    const int len = 8 * min(TX + 2, nx + 2 - x0);
+                    for (int off = 0; off < len; off += 128) prefetch_l2(p0 + off);
+                    prefetch_l2(p0 + len - 8);
+                }
+            } else if (t < 20 * (TY + 2) + 10 * TY) {                // U^n and U_(s) of the cells that the next iteration finishes ... of plane kk
+                const int u = t - 20 * (TY + 2);
+                const int a = u / TY, r = u - a * TY;
+                if (y0 + r < ny) {
+                    const double* base = (a < 5 ? Ua.q[0] : V.q[0]) + (unsigned long long)(a < 5 ? a : a - 5) * (unsigned long long)g.ncell;
+                    const char* p0 = reinterpret_cast<const char*>(base + (unsigned int)x0 + (unsigned int)(y0 + r) * ns1 + (unsigned int)kk * ns2);
+                    const int len = 8 * min(TX, nx - x0);
+                    for (int off = 0; off < len; off += 128) prefetch_l2(p0 + off);
+                    prefetch_l2(p0 + len - 8);
+                }
+            }
+        }
+        // ---------------------------------------------------------------- z interface kk-1/2 of the own column
+        double Fz[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
+        if (cell_ok) {
+            const unsigned int p = cpe + (unsigned int)kk * es2, pn = p + es2;      // extended plane kk holds interior plane kk-1
+            double A[5], B[5];
+#ifdef MF_STRICT
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { A[v] = fc.f[2][1][v][p]; B[v] = fc.f[2][0][v][pn]; }
+#else
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { A[v] = Wc.q[v][p] + fc.f[2][0][v][p]; B[v] = Wc.q[v][pn] - fc.f[2][0][v][pn]; }
+#endif
+            musta_flux<2>(q, k, mcf, A, B, Fz);
+        }
+        if (kk > z0) bar.wait(std::move(token));                     // F_x, F_y of plane kk-1 are complete; buffer `buf` is free again
+        if (cell_ok) {
+            if (kk > z0) {                                           // cell (gx, gy, kk-1) is complete
+                const int kc = kk - 1, pb = buf ^ 1;
+                const unsigned int o = co + (unsigned int)kc * ns2;
+                const double dt = sc.dt;
+                double S = 0.0;
+                if (src.on) S = jet_source(g, src, gx, gy, kc, ds->t + sg.ts * dt);
+                double ua5[5], ub5[5];                               // loaded before the first store (`out` may alias them for all the compiler knows)
+#pragma unroll
+                for (int v = 0; v < 5; ++v) {
+                    ua5[v] = sg.form == 3 ? 0.0 : Ua.q[v][o];
+                    ub5[v] = (sg.form == 1 || sg.form == 2) ? V.q[v][o] : 0.0;
+                }
+                double W[5];
+#pragma unroll
+                for (int v = 0; v < 5; ++v) {
+                    double acc = sFx[pb][v][cj * (TX + 1) + ci + 1] - sFx[pb][v][cj * (TX + 1) + ci];
+                    acc = acc + (sFy[pb][v][(cj + 1) * TX + ci] - sFy[pb][v][cj * TX + ci]);
+                    acc = acc + (Fz[v] - sFz[v][t]);
+#ifdef MF_STRICT
+                    double L = -acc / g.dx;                          // Eq.1 :43
+#else
+                    double L = -acc * g.inv_dx;
+#endif
+                    if (src.on && v < 2) L = L + S;
+                    W[v] = rk_form(sg, ua5[v], ub5[v], dt, L);
+                    out.q[v][o] = W[v];
+                }
+                if (CFL) smax = fmax(smax, signal_speed<0>(q, W[0], W[1], W[2], W[3], W[4], bad));
+            }
+#pragma unroll
+            for (int v = 0; v < 5; ++v) sFz[v][t] = Fz[v];
+        }
+        if (kk == z1) break;                                         // the last pass only closes plane z1-1
+        // ---------------------------------------------------------------- x and y interfaces of plane kk
+        const unsigned int pz = (unsigned int)(kk + 1) * es2;
+        if (xtask) {
+            const unsigned int p = xp + pz;
+            double A[5], B[5], F[5];
+#ifdef MF_STRICT
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { A[v] = fc.f[0][1][v][p]; B[v] = fc.f[0][0][v][p + 1]; }
+#else
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { A[v] = Wc.q[v][p] + fc.f[0][0][v][p]; B[v] = Wc.q[v][p + 1] - fc.f[0][0][v][p + 1]; }
+#endif
+            musta_flux<0>(q, k, mcf, A, B, F);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) sFx[buf][v][t] = F[v];
+        }
+        if (ytask) {
+            const unsigned int p = yp + pz, pn = p + es1;
+            double A[5], B[5], F[5];
+#ifdef MF_STRICT
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { A[v] = fc.f[1][1][v][p]; B[v] = fc.f[1][0][v][pn]; }
+#else
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { A[v] = Wc.q[v][p] + fc.f[1][0][v][p]; B[v] = Wc.q[v][pn] - fc.f[1][0][v][pn]; }
+#endif
+            musta_flux<1>(q, k, mcf, A, B, F);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) sFy[buf][v][t] = F[v];
+        }
+        token = bar.arrive();
+    }
+    if (CFL) block_reduce_smax<NT>(smax, bad, ds);
+}
+
 static int tile_chunk(const Grid& g, int ntx, int nty, int num_sms)
 {
     // z chunk: all of z, or the largest of {64, 32, 16, 8} planes for which the items fill the 3 resident CTA slots per SM ~6 times over
@@ -289,16 +454,24 @@ int launch_tile_stage(const Grid& g, const Eos& q, int limiter, int predictor, i
 
 // hybrid: face states come from k_cell_stage's scratch (fc); the tile kernel does the three flux directions and the combine
 int launch_tile_stage_pre(const Grid& g, const Eos& q, int k, Faces fc, CState5 V, Stage sg, CState5 Ua, State5 out, Source src,
-                          const StepState* ds, int num_sms, cudaStream_t st)
+                          StepState* ds, int num_sms, cudaStream_t st)
 {
     const int ntx = (g.n[0] + TX - 1) / TX, nty = (g.n[1] + TY - 1) / TY;
     const int TZ = tile_chunk(g, ntx, nty, num_sms);
     const unsigned int grid = (unsigned int)(ntx * nty * ((g.n[2] + TZ - 1) / TZ));
-    const size_t smem = sizeof(double) * 35 * NT;
-    static DeviceOnce once;
-    if (once.first()) cudaFuncSetAttribute(k_tile_stage<LIM_NONE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    k_tile_stage<LIM_NONE, true><<<grid, NT, smem, st>>>(g, q, 0, k, TZ, ntx, nty, V, V, fc, sg, Ua, out, src, ds);
+    CState5 Wc;
+    for (int v = 0; v < 5; ++v) Wc.q[v] = fc.f[0][1][v];
+    if (g.cslot >= 0) {
+        if (sg.cfl) k_tile3<true, true><<<grid, NT, 0, st>>>(g, q, k, TZ, ntx, nty, fc, Wc, V, sg, Ua, out, src, ds);
+        else k_tile3<false, true><<<grid, NT, 0, st>>>(g, q, k, TZ, ntx, nty, fc, Wc, V, sg, Ua, out, src, ds);
+    } else {
+        if (sg.cfl) k_tile3<true, false><<<grid, NT, 0, st>>>(g, q, k, TZ, ntx, nty, fc, Wc, V, sg, Ua, out, src, ds);
+        else k_tile3<false, false><<<grid, NT, 0, st>>>(g, q, k, TZ, ntx, nty, fc, Wc, V, sg, Ua, out, src, ds);
+    }
     return 1;
 }
+
+int upload_step_const_tile(const StepConst* dsc, int slot, int nev, cudaStream_t st) { return upload_step_const(dsc, slot, nev, st); }
+bool tile_reduces_cfl() { return true; }
 
 } // namespace mf
