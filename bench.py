@@ -42,30 +42,39 @@ DIV, SQRT = 8, 8
 FLUX = 16 + DIV + SQRT                    # a6: one flux evaluation with con2prim             = 32
 DIV_MIN, SQRT_MIN, FLUX_MIN = 3, 6, 24
 SLOPE = {"none": 2, "first": 0, "minmod": 3, "superbee": 7, "mc": 8, "vanleer": 4 + DIV, "vanalbada": 6 + DIV}
+# Tabulated EOS (8(f) row 1): a flux evaluation is the 16 slots of the flux arithmetic plus one speed solve.  Measured on this workload with the
+# counting build (-DMF_COUNT_EVALS: 1.84e9 solves at 128^3, one full table evaluation and 0.00 incremental ones per solve, no fallback): the
+# fp32-seeded Newton reaches its stopping rule after ONE fp64 evaluation, ~185 FP64 instructions per solve (root 6, three reciprocals 9, log ~20,
+# exp ~20, bilinear lookup with derivatives ~25, Newton step and the first-order pressure update ~20, admissibility and cell test ~20, the rest
+# in the guard), so the algorithmic count is 16 + 185 = 201 slots in both conventions (its root and reciprocals are already the minimal ones).
+FLUX_TABLE = 16 + 185
 SLOPE_MIN = {"none": 2, "first": 0, "minmod": 3, "superbee": 7, "mc": 8, "vanleer": 4 + DIV_MIN, "vanalbada": 6 + DIV_MIN}
 
 
-def alg_slots(limiter, k, rk, ndim, predictor=True, minimal=False):
+def alg_slots(limiter, k, rk, ndim, predictor=True, minimal=False, table=False):
     """(slots per cell-update, slots per L-evaluation, slots of the MUSTA fluxes per L-evaluation)."""
     flux, div, sqrt, slope = (FLUX_MIN, DIV_MIN, SQRT_MIN, SLOPE_MIN) if minimal else (FLUX, DIV, SQRT, SLOPE)
+    if table:
+        flux = FLUX_TABLE
     recon = 5 * ndim * (4 + slope[limiter])                         # a3: a, b, slope, two face values
     pred = (2 * ndim * flux + 5 * 4 * ndim) if predictor else 0     # a4: 2D flux evaluations + delta + 2D face updates
     force = 3 * flux + 50                                           # Eq.9-11: three fluxes + 10 per component
     musta = (k + 1) * force + 20 * k                                # a5: k Eq.8 updates
     comb = 5 * (2 * ndim + 5)                                       # a7: divergence + RK form
-    cfl = (16 + div + sqrt) + (3 + sqrt) + (2 + div) + 1            # a2
+    cfl = ((FLUX_TABLE + 60) if table else (16 + div + sqrt)) + (3 + sqrt) + (2 + div) + 1     # a2 (table: one more lookup for the sound speed)
     per_L = recon + pred + ndim * musta + comb
     return rk * per_L + cfl, per_L, ndim * musta
 
 
-def class_work(path, limiter, k, ndim, x_active, predictor=True, state_bytes=8):
+def class_work(path, limiter, k, ndim, x_active, predictor=True, state_bytes=8, table=False):
     """Algorithmic (FP64 slots, HBM bytes) per cell of one launch group of each kernel class, for one RK stage.
     Bytes are what that kernel must read and write given the data layout of DESIGN.md section 4; `state_bytes` is the size of a stored
     state element (8, or 4 in single-precision state mode, staged path only: the scratch stays fp64)."""
     sb = 5 * state_bytes                                                       # one state, per cell
+    fl = FLUX_TABLE if table else FLUX
     recon = 5 * ndim * (4 + SLOPE[limiter])
-    pred = (2 * ndim * FLUX + 5 * 4 * ndim) if predictor else 0
-    musta = (k + 1) * (3 * FLUX + 50) + 20 * k
+    pred = (2 * ndim * fl + 5 * 4 * ndim) if predictor else 0
+    musta = (k + 1) * (3 * fl + 50) + 20 * k
     comb = 5 * (2 * ndim + 5)
     if path == "staged":
         nflux = ndim - 1 if x_active else ndim
@@ -353,11 +362,12 @@ def run_ours(args):
     pk = peaks()
     pred_on = sch.get("predictor", True)
     state_bytes = 4 if args.state == "f32" else 8
-    slots_cu, slots_L, slots_musta = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim, pred_on)
-    slots_cu_min = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim, pred_on, minimal=True)[0]
+    table = args.eos == "table"
+    slots_cu, slots_L, slots_musta = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim, pred_on, table=table)
+    slots_cu_min = alg_slots(sch["limiter"], sch["k_stages"], sch["rk"], ndim, pred_on, minimal=True, table=table)[0]
     alu_peak_slots = 148 * FP64_LANES_PER_SM * pk["sm_max_mhz"] * 1e6          # FP64 instructions/s, all SMs
     # dominant kernel, from the event pairs recorded around every launch inside the timed region
-    work = class_work(g.path(), sch["limiter"], sch["k_stages"], ndim, nx > 1, pred_on, state_bytes)
+    work = class_work(g.path(), sch["limiter"], sch["k_stages"], ndim, nx > 1, pred_on, state_bytes, table)
     kernels = {}
     for name, (ms, groups) in prof.items():
         if name not in work or groups == 0:
@@ -403,7 +413,9 @@ def run_ours(args):
                                     "single-precision STATE (PAPER.md:250, reading A19; arithmetic and scratch stay fp64) - outside "
                                     "BASELINE.json's fp64 contract, reported beside the headline, never as it",
                                     "status": status, "eos": "p = e/3 (closed-form con2prim)" if args.eos == "cs2" else
-                                    "tabulated crossover p(e,n), Newton con2prim (roofline fractions below use the closed-form slot count)"}),
+                                    "tabulated crossover p(e,n), Newton con2prim (roofline: 201 slots per flux evaluation = 16 + one speed solve of ~185 FP64 "
+                                    "instructions, one full table evaluation per solve measured with the counting build; the kernels are bound by "
+                                    "instruction issue - fp32 seed, table addressing, call overhead - not by the FP64 pipe)"}),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 40 * cells, "d2h_bytes_per_step": 40 * cells,
                     "steps": e2e_steps, "note": "mf_set_state(host) + mf_step(1) + mf_get_state(host) per step, pinned host buffers"},

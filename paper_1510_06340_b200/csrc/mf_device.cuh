@@ -98,6 +98,14 @@ __device__ __forceinline__ EosValue eos_eval(const Eos& q, double e, double n)
 struct SpeedEP {
     double v, e, p;
 };
+// Measurement build only (-DMF_COUNT_EVALS, never the product): how many speed solves run and how many table evaluations they take,
+// printed by k_end_step; bench.py's roofline for the tabulated EOS is built on these means (DESIGN.md section 10 row 1).
+#ifdef MF_COUNT_EVALS
+static __device__ unsigned long long g_eval_count[4];      // solves, full evaluations (log + exp), incremental evaluations, fallback solves
+#define MF_COUNT(i) atomicAdd(&g_eval_count[i], 1ull)
+#else
+#define MF_COUNT(i) ((void)0)
+#endif
 #ifndef MF_STRICT
 // ---- product build: the same root in far fewer FP64 instructions.
 //  1. fp32 seed: the p = e/3 closed form, then two Newton steps on the float copy of the table (MUFU log/exp): |dv|/v ~ 1e-5.
@@ -220,7 +228,7 @@ __device__ __forceinline__ bool solve_speed_fast(const TableRef& q, double E, do
     for (int it = 0; it < 6; ++it) {
         const double e = fma(-M, v, E);
         const double g = sqrt_newton(fma(-v, v, 1.0));
-        if (it == 0) table_eval_step<false>(q, e, R * g, s); else table_eval_step<true>(q, e, R * g, s);
+        if (it == 0) { MF_COUNT(1); table_eval_step<false>(q, e, R * g, s); } else { MF_COUNT(2); table_eval_step<true>(q, e, R * g, s); }
         const double f = fma(v, E + s.p, -M);
         const double dpdv = -fma(M, s.p_e, R * (v * rcp_pos(g)) * s.p_n);
         const double df = fma(v, dpdv, E + s.p);
@@ -251,12 +259,14 @@ __device__ __forceinline__ bool solve_speed_fast(const TableRef& q, double E, do
 
 static __device__ __noinline__ SpeedEP solve_speed(TableRef q, double E, double M, double R)
 {
+    MF_COUNT(0);
 #ifndef MF_STRICT
     {
         SpeedEP r;
         if (solve_speed_fast(q, E, M, R, r.v, r.e, r.p)) return r;
     }
 #endif
+    MF_COUNT(3);
     double lo = 0.0, hi = M / E, v = hi;
     for (int it = 0; it < 60; ++it) {
         const double e = E - M * v;
@@ -368,10 +378,18 @@ __device__ __forceinline__ void velocity_pressure(const Eos& q, double E, double
         M2 = Mx * Mx + My * My + Mz * Mz;
     }
     if (EK != 0) {                                // tabulated EOS: Newton on the speed, then v_j = M_j v/|M|
+#ifdef MF_STRICT
         const double M = sqrt(M2);
+#else
+        const double M = M2 > 1e-280 ? sqrt_pos(M2) : sqrt(M2);            // (Newton root: normal, positive arguments only)
+#endif
         if (M == 0.0) { vx = vy = vz = 0.0; e = E; p = eos_table_eval(table_of(q), E, R).p; return; }
         const SpeedEP r = solve_speed(table_of(q), E, M, R);
+#ifdef MF_STRICT
         const double s = r.v / M;
+#else
+        const double s = M > 1e-140 ? r.v * rcp_pos(M) : r.v / M;
+#endif
         vx = Mx * s; vy = My * s; vz = Mz * s; e = r.e; p = r.p;
         return;
     }

@@ -2,6 +2,7 @@
 // CFL reduction (a2), per-step scalars, cell stage (a3+a4), interface flux stage (a5+a6), combine (a7+a8),
 // prim<->con conversions, totals.  Boundary handling (a1) is index mapping in the loads: no stored ghosts.
 #include "mf_kernels.h"
+#include <cstdio>
 #include "mf_blocks.cuh"
 #include "mf_stepconst.cuh"
 
@@ -97,6 +98,10 @@ __global__ void k_end_step(StepState* ds, int nev)
     ds += ev;
     ds->t = ds->t + ds->dt;
     ds->steps += 1;
+#ifdef MF_COUNT_EVALS
+    if (ev == 0) printf("MF_COUNT_EVALS step %lld: solves %llu full %llu incremental %llu fallback %llu\n", ds->steps, g_eval_count[0], g_eval_count[1],
+                        g_eval_count[2], g_eval_count[3]);
+#endif
 }
 
 __global__ void k_reset(StepState* ds, int nev)
