@@ -1,6 +1,13 @@
-// mf_tile.cu — fused path, tile kernel (one launch per RK stage after k_delta_stage): a1, a3, a5, a6, a7, a8 on chip.
+// mf_tile.cu — the two tile kernels (3D grids, p = cs2*e, one event):
 //
-// A CTA of 256 threads owns a tile of 32 x 7 cells in (x, y) and marches through a chunk of z planes.  Work inside the CTA is a
+//   k_tile3      (MF_PATH_HYBRID, round 2): fed by the staged cell stage's scratch (W = U + delta, half slopes); a CTA of 256 threads owns
+//                32 x 7 cells and marches in z; every x, y and z interface is a TASK of one thread, which loads its own operands from
+//                global memory (L1/L2, the next plane prefetched line by line) and runs MUSTA; only the finished fluxes go through shared
+//                memory; divergence, source, RK combine and the CFL reduction of plane k-1 follow the z interface that completes it; ONE
+//                split barrier per plane.  See the comment above the kernel.
+//   k_tile_stage (MF_PATH_FUSED, round 1): one launch per RK stage after k_delta_stage: a1, a3, a5, a6, a7, a8 on chip.
+//
+// k_tile_stage: a CTA of 256 threads owns a tile of 32 x 7 cells in (x, y) and marches through a chunk of z planes.  Work inside the CTA is a
 // pool of INTERFACE TASKS, not a thread-per-cell map, so that no thread idles on a ring cell.  Per plane kk:
 //   cell parts : 34 x 7 threads rebuild the x face states U~xL, U~xR of the tile's cells and of the two ring cells of each row,
 //                32 x 9 threads the y face states (U -/+ slope/2 + delta: a dozen FP64 instructions per component), and drop them
