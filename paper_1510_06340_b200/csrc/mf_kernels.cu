@@ -294,12 +294,13 @@ int launch_cell_stage(const Grid& g, const Eos& q, int limiter, int predictor, C
 // =========================================================================== a5 + a6: interface fluxes
 // One thread per interface between cell c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
 template <int D, int EK, bool UC>
-__global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, int k, CState5 Wc, Faces fc, Fluxes fx, const StepState* ds)
+__device__ __forceinline__ void flux_stage_body(const Grid& g, const Eos& q, int k, const CState5& Wc, const Faces& fc, const Fluxes& fx,
+                                                const StepState* ds, unsigned int block)
 {
     int m[3] = { g.n[0], g.n[1], g.n[2] };
     m[D] += 1;
     const long long total = (long long)m[0] * m[1] * m[2];
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long t = (long long)block * blockDim.x + threadIdx.x;
     if (t >= total) return;
     int c[3];
     unflatten3((unsigned int)t, g.dv[0][D == 0], g.dv[1][D == 1], c[0], c[1], c[2]);
@@ -322,11 +323,36 @@ __global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, 
     for (int v = 0; v < 5; ++v) fx.f[D][v][p] = F[v];
 }
 
+template <int D, int EK, bool UC>
+__global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, int k, CState5 Wc, Faces fc, Fluxes fx, const StepState* ds)
+{
+    flux_stage_body<D, EK, UC>(g, q, k, Wc, fc, fx, ds, blockIdx.x);
+}
+
+// The y and the z interfaces of a stage are independent of each other: ONE launch runs both (blocks [0, nby) take y, the rest z), so that the
+// z blocks fill the SMs while the last y blocks drain - one kernel boundary less per RK stage.
+template <int EK, bool UC>
+__global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage_yz(Grid g, Eos q, int k, CState5 Wc, Faces fc, Fluxes fx, const StepState* ds, unsigned int nby)
+{
+    if (blockIdx.x < nby) flux_stage_body<1, EK, UC>(g, q, k, Wc, fc, fx, ds, blockIdx.x);
+    else flux_stage_body<2, EK, UC>(g, q, k, Wc, fc, fx, ds, blockIdx.x - nby);
+}
+
 int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, Fluxes fx, const StepState* ds, cudaStream_t st)
 {
     int launches = 0;
     CState5 Wc;
     for (int v = 0; v < 5; ++v) Wc.q[v] = fc.f[g.act[0] ? 0 : (g.act[1] ? 1 : 2)][1][v];
+#ifndef MF_NO_YZ_MERGE
+    if (dmask == 6 && g.act[1] && g.act[2]) {
+        const unsigned int nby = blocks_for((long long)g.n[0] * (g.n[1] + 1) * g.n[2], FT), nbz = blocks_for((long long)g.n[0] * g.n[1] * (g.n[2] + 1), FT);
+        const dim3 nb(nby + nbz, g.nev);
+        if (q.kind) k_flux_stage_yz<1, false><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds, nby);
+        else if (g.cslot >= 0) k_flux_stage_yz<0, true><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds, nby);
+        else k_flux_stage_yz<0, false><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds, nby);
+        return 1;
+    }
+#endif
     for (int d = 0; d < 3; ++d) {
         if (!g.act[d] || !(dmask & (1 << d))) continue;
         long long total = 1;
