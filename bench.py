@@ -186,6 +186,16 @@ def make_workload(args):
     st = workloads.gaussian_hot_spot() if (args.config == 3 and shape is None) else workloads.config(args.config, scale=shape)
     if args.predictor == "off":
         st["scheme"] = dict(st["scheme"], predictor=False)
+    over = {}
+    if args.k is not None:
+        over["k_stages"] = args.k
+    if args.limiter is not None:
+        over["limiter"] = args.limiter
+    if args.rk is not None:
+        over["rk"] = args.rk
+    if over:                                                   # not a BASELINE.json config any more: say so in the workload name
+        st["scheme"] = dict(st["scheme"], **over)
+        st["name"] = st["name"] + " (scheme overridden: %s)" % ", ".join("%s=%s" % kv for kv in sorted(over.items()))
     return st
 
 
@@ -450,6 +460,9 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid", "sweep"])
     ap.add_argument("--eos", default="cs2", choices=["cs2", "table"], help="table: synthetic crossover p(e,n) table with Newton con2prim")
     ap.add_argument("--predictor", default="on", choices=["on", "off"], help="off: without the Hancock half step (reading A4), reported beside the default")
+    ap.add_argument("--k", type=int, default=None, help="override the number of MUSTA stages (e.g. 4: the paper's own setting, PAPER.md:256)")
+    ap.add_argument("--limiter", default=None, choices=["none", "minmod", "superbee", "vanalbada", "vanleer", "mc", "first"])
+    ap.add_argument("--rk", type=int, default=None, choices=[2, 3])
     ap.add_argument("--state", default="f64", choices=["f64", "f32"],
                     help="f32: single-precision stored state (PAPER.md:250, reading A19), staged path; not the headline")
     ap.add_argument("--batch", type=int, default=1, help="events per context (mf_create_batch); config 4: the seeded events 0..B-1")

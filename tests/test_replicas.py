@@ -80,3 +80,14 @@ def test_algorithmic_work_matches_survey_table():
     assert m22 == 3 * 478 and m33 == 3 * 644
     assert 3500 <= s22 <= 3800 and 7000 <= s33 <= 7400
     assert bench.alg_bytes(2) == 232 and bench.alg_bytes(3) == 352
+    # the second convention (the sequences the product code issues: reciprocal 3, root 6, flux 24) is below the survey's and counts the same
+    # pieces: per MUSTA interface (k+1)(3*24 + 50) + 20k
+    n33, _, mm33 = bench.alg_slots("superbee", 3, 3, 3, minimal=True)
+    assert mm33 == 3 * (4 * (3 * 24 + 50) + 60) and n33 < s33 and 6000 <= n33 <= 6500
+    # single-precision state: the state's bytes halve, the slots do not change
+    assert bench.alg_bytes(3, state_bytes=4) == 176
+    # tabulated EOS: 201 slots per flux evaluation in both conventions (they differ only in the root and divide of the CFL pass)
+    t33 = bench.alg_slots("superbee", 3, 3, 3, table=True)[0]
+    assert abs(t33 - bench.alg_slots("superbee", 3, 3, 3, table=True, minimal=True)[0]) < 20 and t33 > 3 * s33
+    w = bench.class_work("staged", "superbee", 3, 3, True, True, state_bytes=4)
+    assert w["cell_stage"][1] == 20 + 160 and w["combine"][1] == 160 + 60
