@@ -79,6 +79,14 @@ int mf_batch_size(mf_ctx*);                 /* nevents (1 for mf_create) */
 int mf_set_state(mf_ctx*, const double* E, const double* Mx, const double* My, const double* Mz, const double* R);
 /* Copy the conserved state out (5 HOST arrays).  Synchronises; returns MF_ESTATE if the sticky flag is up. */
 int mf_get_state(mf_ctx*, double* E, double* Mx, double* My, double* Mz, double* R);
+/* The same two copies WITHOUT synchronisation, for callers that stream independent events through several contexts (upload the next
+ * event and download the last result while the current one is being stepped; event-by-event running is what the paper builds its code for,
+ * :25, :389): the copies are enqueued on the context's stream and the call returns.  The HOST arrays must be page-locked (pinned) for the
+ * copies to overlap with anything, must stay valid and untouched until the stream has passed them - mf_sync(ctx) or any synchronising call -
+ * and the arrays of mf_get_state_async hold the state only after that.  Contexts are independent (one stream each), so set/step/get of
+ * one context overlap with those of another.  The sticky state flag is reported by the next synchronising call, not here. */
+int mf_set_state_async(mf_ctx*, const double* E, const double* Mx, const double* My, const double* Mz, const double* R);
+int mf_get_state_async(mf_ctx*, double* E, double* Mx, double* My, double* Mz, double* R);
 /* Same with DEVICE arrays; ordered on the context's stream, set does not synchronise. */
 int mf_set_state_device(mf_ctx*, const double* E, const double* Mx, const double* My, const double* Mz, const double* R);
 int mf_get_state_device(mf_ctx*, double* E, double* Mx, double* My, double* Mz, double* R);

@@ -30,6 +30,8 @@ SIGNATURES = {
     "mf_destroy": (None, [_vp]),
     "mf_set_state": (C.c_int, [_vp] + _d5),
     "mf_get_state": (C.c_int, [_vp] + _d5),
+    "mf_set_state_async": (C.c_int, [_vp] + _d5),
+    "mf_get_state_async": (C.c_int, [_vp] + _d5),
     "mf_set_state_device": (C.c_int, [_vp] + _v5),
     "mf_get_state_device": (C.c_int, [_vp] + _v5),
     "mf_set_state_prim": (C.c_int, [_vp] + _d5),
@@ -245,6 +247,20 @@ class MustaForce:
         nn, ne = (1, ln_p.size) if ln_p.ndim == 1 else ln_p.shape
         self._chk(self.lib.mf_set_eos_table(self.h, ne, nn, float(tb["ln_e0"]), float(tb["dln_e"]), float(tb.get("n0", 0.0)),
                                             float(tb.get("dn", 1.0)), _p(ln_p)))
+
+    def set_state_async(self, E, Mx, My, Mz, R):
+        """No synchronisation: the five float64 arrays (pinned, contiguous, of the context's size) must stay alive and untouched until sync()."""
+        for x in (E, Mx, My, Mz, R):
+            if x.dtype != np.float64 or not x.flags["C_CONTIGUOUS"] or x.size != self.n:
+                raise ValueError("set_state_async needs contiguous float64 arrays of %d elements (no copy can be made here)" % self.n)
+        self._chk(self.lib.mf_set_state_async(self.h, *[_p(x) for x in (E, Mx, My, Mz, R)]))
+
+    def get_state_async(self, out):
+        """Enqueue the copy of the state into the five (pinned) float64 arrays `out`; they are complete after sync()."""
+        for x in out:
+            if x.dtype != np.float64 or not x.flags["C_CONTIGUOUS"] or x.size != self.n:
+                raise ValueError("get_state_async needs contiguous float64 arrays of %d elements" % self.n)
+        self._chk(self.lib.mf_get_state_async(self.h, *[_p(x) for x in out]))
 
     def set_stream(self, stream):
         """stream: a raw cudaStream_t as int (e.g. torch.cuda.current_stream().cuda_stream); 0/None = own stream."""

@@ -636,6 +636,27 @@ int mf_set_state(mf_ctx* c, const double* E, const double* Mx, const double* My,
     return MF_OK;
 }
 
+int mf_set_state_async(mf_ctx* c, const double* E, const double* Mx, const double* My, const double* Mz, const double* R)
+{
+    if (!c) return MF_EINVAL;
+    if (!E || !Mx || !My || !Mz || !R) return fail(c, MF_EINVAL, "null pointer");
+    const double* src[5] = { E, Mx, My, Mz, R };
+    int rc = copy_in(c, src, cudaMemcpyHostToDevice);
+    if (rc != MF_OK) return rc;
+    finish_copy_in(c);
+    return reset_after_set(c);                                     // no synchronisation: the host arrays stay in use until the stream has passed
+}
+
+int mf_get_state_async(mf_ctx* c, double* E, double* Mx, double* My, double* Mz, double* R)
+{
+    if (!c) return MF_EINVAL;
+    if (!E || !Mx || !My || !Mz || !R) return fail(c, MF_EINVAL, "null pointer");
+    double* dst[5] = { E, Mx, My, Mz, R };
+    int rc = copy_out(c, state_as_doubles(c), dst, cudaMemcpyDeviceToHost);
+    if (rc != MF_OK) return rc;
+    return check_launch(c);                                        // the arrays are complete after the next mf_sync
+}
+
 int mf_set_state_device(mf_ctx* c, const double* E, const double* Mx, const double* My, const double* Mz, const double* R)
 {
     if (!c) return MF_EINVAL;

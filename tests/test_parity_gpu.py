@@ -240,6 +240,34 @@ def test_device_pointer_state_io_and_user_stream():
     assert g.launch_count() > 0
 
 
+def test_async_state_io_streams_events_through_several_contexts():
+    """mf_set_state_async / mf_get_state_async: three contexts on their own streams, events handed round-robin with pinned buffers; every
+    event's result equals the synchronous calls' bit for bit, and the buffers are complete after mf_sync."""
+    import torch
+    events = [w.lumpy_event(event=e, shape=(12, 14, 16), dx=0.3) for e in range(7)]
+    F = ("E", "Mx", "My", "Mz", "R")
+    ctxs = [MustaForce(16, 14, 12, dx=0.3, limiter="mc", k_stages=2, rk=3) for _ in range(3)]
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    ins = [[pin(ev[f]) for f in F] for ev in events]
+    outs = [[pin(np.zeros_like(ev["E"])) for _ in F] for ev in events]
+    for i, ev in enumerate(events):
+        c = ctxs[i % 3]
+        assert c.sync() == 0                                               # its previous event is complete
+        c.set_state_async(*ins[i])
+        c.step(4, 0.3)
+        c.get_state_async(outs[i])
+    for c in ctxs:
+        assert c.sync() == 0
+    ref = MustaForce(16, 14, 12, dx=0.3, limiter="mc", k_stages=2, rk=3)
+    for i, ev in enumerate(events):
+        ref.set_state(*[ev[f] for f in F])
+        ref.step(4, 0.3)
+        for a, b in zip(outs[i], ref.get_state()):
+            assert np.array_equal(a, b)
+    with pytest.raises(ValueError):
+        ctxs[0].set_state_async(*[x.astype(np.float32) for x in ins[0]])
+
+
 # ------------------------------------------------------------------ full-size grids: windowed parity (DESIGN.md "Parity at full size")
 def _windowed_parity(st, centre, steps_before=95, m=5, half=8, path="auto"):
     """Advance the FULL grid on the GPU to step steps_before, then re-run the last m steps with the oracle on a sub-box around `centre`
