@@ -90,8 +90,8 @@ def class_work(path, limiter, k, ndim, x_active, predictor=True, state_bytes=8, 
         # separate kernel writes delta (the reconstruction is then counted once more there: it is needed for Eq.13)
         rdir = recon // ndim
         dl = 40 if predictor else 0
-        out = {"flux_stage": ((ndim - 1) * (musta + rdir), (ndim - 1) * (40 + dl + 40)),          # U (+ delta) in, F_d out
-               "combine": (musta + rdir + comb, 40 + dl + 40 * (ndim - 1) + 40 + 40)}            # U (+ delta), F_y, F_z, U^n in; new state out
+        out = {"flux_stage": ((ndim - 1) * (musta + rdir), (ndim - 1) * (sb + dl + 40)),          # U (+ delta) in, F_d out
+               "combine": (musta + rdir + comb, sb + dl + 40 * (ndim - 1) + sb + sb)}            # U (+ delta), F_y, F_z, U^n in; new state out
         if predictor:
             out["cell_stage"] = (recon + pred, 80)                                                 # U in, delta out
         return out

@@ -136,8 +136,8 @@ int mf_set_low_storage(mf_ctx*, int on);
  * stage are rounded to nearest even on the store - while all arithmetic between a load and the next store, the scratch (face states, fluxes)
  * and the CFL reduction (taken from the stored, rounded U^n) stay fp64.  Halves the bytes of the state registers that cross HBM.  The calls
  * that hand states in or out keep their double arrays (values are rounded on the way in and widened on the way out).  bits = 64 (default)
- * restores the fp64 state.  The current state is converted; synchronises.  Staged path only (MF_PATH_AUTO then resolves to it); MF_EINVAL for
- * another bit count or if another path is selected.  Outside BASELINE.json's fp64 contract: bench.py reports it beside the headline, never as it. */
+ * restores the fp64 state.  The current state is converted; synchronises.  Runs on the staged path and, without the Hancock predictor, on
+ * the sweep path (MF_PATH_AUTO resolves accordingly); MF_EINVAL for another bit count or if a path that cannot carry it is selected.  Outside BASELINE.json's fp64 contract: bench.py reports it beside the headline, never as it. */
 int mf_set_state_precision(mf_ctx*, int bits);
 int mf_get_state_precision(mf_ctx*, int* bits);
 /* mf_step / mf_step_dt replay whole steps from a CUDA graph when n >= 7 (5 in low-storage mode): one eager step, then one captured period of

@@ -162,9 +162,12 @@ void clear_table(Eos& q)
 int resolve_path(mf_ctx* c)
 {
     if (c->g.state32) {
-        // single-precision state: the kernels of the staged path carry the state element type (the sweep and tile kernels read doubles)
+        // single-precision state: the kernels of the staged path and, without the Hancock step, of the sweep path carry the state element
+        // type (k_delta_stage and the tile kernels read doubles)
+        const bool sweep_ok = !c->predictor && c->nreg == 3 && sweep_supported(c->g, c->q.kind || c->eos != MF_EOS_CS2, 0);
+        if (c->path_req == MF_PATH_SWEEP) { if (!sweep_ok) return MF_EINVAL; c->path = MF_PATH_SWEEP; return MF_OK; }
         if (c->path_req != MF_PATH_AUTO && c->path_req != MF_PATH_STAGED) return MF_EINVAL;
-        c->path = MF_PATH_STAGED;
+        c->path = (c->path_req == MF_PATH_AUTO && sweep_ok) ? MF_PATH_SWEEP : MF_PATH_STAGED;
         return MF_OK;
     }
     if (c->nreg == 2) {
@@ -274,7 +277,9 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
         if (rc != MF_OK) return rc;
         Fluxes fx = fluxes_of(c);
         const bool pred = c->predictor != 0;
-        CState5 Dl = cstate(pred ? c->delta : V, pred ? c->g.next : n);
+        const CState5 Vs = creg(c, V), Uas = creg(c, Ua);
+        const State5 outs = sg.form == 3 ? state(out, n) : reg(c, out);
+        CState5 Dl = pred ? cstate(c->delta, c->g.next) : Vs;
         int ps;
         if (pred) {
             ps = prof_begin(c, 1);
@@ -283,11 +288,11 @@ int run_stage(mf_ctx* c, const double* V, const Stage& sg, const double* Ua, dou
         }
         if (c->g.act[1] || c->g.act[2]) {
             ps = prof_begin(c, 2);
-            c->launches += launch_sweep_flux(c->g, c->q, c->limiter, c->k, pred, cstate(V, n), Dl, fx, c->ds, c->stream);
+            c->launches += launch_sweep_flux(c->g, c->q, c->limiter, c->k, pred, Vs, Dl, fx, c->ds, c->stream);
             prof_end(c, ps);
         }
         ps = prof_begin(c, 3);
-        c->launches += launch_sweep_xcombine(c->g, c->q, c->limiter, c->k, pred, cstate(V, n), Dl, fx, sg, cstate(Ua, n), state(out, n), c->src, c->ds, c->stream);
+        c->launches += launch_sweep_xcombine(c->g, c->q, c->limiter, c->k, pred, Vs, Dl, fx, sg, Uas, outs, c->src, c->ds, c->stream);
         prof_end(c, ps);
     } else {
         int rc = ensure_staged_buffers(c);
@@ -1039,7 +1044,7 @@ int mf_set_state_precision(mf_ctx* c, int bits)
     c->g.state32 = on;
     if (resolve_path(c) != MF_OK) {
         c->g.state32 = keep; resolve_path(c);
-        return fail(c, MF_EINVAL, "the single-precision state runs on the staged path only: select MF_PATH_AUTO or MF_PATH_STAGED first");
+        return fail(c, MF_EINVAL, "the single-precision state runs on the staged path and, without the Hancock step, on the sweep path: select MF_PATH_AUTO or MF_PATH_STAGED first");
     }
     // the stored state changes its element type: U^n is converted into the next register (free between steps), which becomes U^n
     const int next = (c->cur + 1) % c->nreg;

@@ -64,7 +64,7 @@ __device__ __forceinline__ void halo4(int c, int n, int periodic, unsigned int s
 
 // =========================================================================== a1 + a3 + a5 + a6 along y or z
 // One thread per interface between cells c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
-template <int D, bool PRED>
+template <int D, bool PRED, class ST>
 __global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, int k, CState5 V, CState5 Dl, Fluxes fx, const StepState* ds)
 {
     int m[3] = { g.n[0], g.n[1], g.n[2] };
@@ -88,7 +88,10 @@ __global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, i
     {
         double um[5], u0[5], u1[5], u2[5];
 #pragma unroll
-        for (int v = 0; v < 5; ++v) { um[v] = __ldg(&V.q[v][o[0]]); u0[v] = __ldg(&V.q[v][o[1]]); u1[v] = __ldg(&V.q[v][o[2]]); u2[v] = __ldg(&V.q[v][o[3]]); }
+        for (int v = 0; v < 5; ++v) {
+            const ST* Vv = reinterpret_cast<const ST*>(V.q[v]);                  // state element type (reading A19): widened on the load
+            um[v] = (double)__ldg(Vv + o[0]); u0[v] = (double)__ldg(Vv + o[1]); u1[v] = (double)__ldg(Vv + o[2]); u2[v] = (double)__ldg(Vv + o[3]);
+        }
         face_pair_rt(lim, um, u0, u1, u2, A, B);
     }
     if (PRED) {                                                              // Eq.13: the same increment on every face of a cell (A3)
@@ -111,7 +114,7 @@ __global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, i
 #define MF_XB 5
 #endif
 constexpr int XT = MF_XT, XB = MF_XB;                // threads per block of the x sweep, blocks per SM (96 registers: the combine holds its operands across the barrier)
-template <bool PRED, int FORM, bool CFL>
+template <bool PRED, int FORM, bool CFL, class ST>
 __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int lim, int k, CState5 V, CState5 Dl, Fluxes fx, Stage sg, CState5 Ua,
                                                            State5 out, Source src, StepState* ds)
 {
@@ -136,7 +139,10 @@ __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int li
         {
             double um[5], u0[5], u1[5], u2[5];
 #pragma unroll
-            for (int v = 0; v < 5; ++v) { um[v] = __ldg(&V.q[v][o[0]]); u0[v] = __ldg(&V.q[v][o[1]]); u1[v] = __ldg(&V.q[v][o[2]]); u2[v] = __ldg(&V.q[v][o[3]]); }
+            for (int v = 0; v < 5; ++v) {
+            const ST* Vv = reinterpret_cast<const ST*>(V.q[v]);                  // state element type (reading A19): widened on the load
+            um[v] = (double)__ldg(Vv + o[0]); u0[v] = (double)__ldg(Vv + o[1]); u1[v] = (double)__ldg(Vv + o[2]); u2[v] = (double)__ldg(Vv + o[3]);
+        }
             face_pair_rt(lim, um, u0, u1, u2, A, B);
         }
         if (PRED) {
@@ -157,8 +163,8 @@ __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int li
         for (int v = 0; v < 5; ++v) {
             if (g.act[1]) { fy1[v] = fx.f[1][v][pc]; fy0[v] = fx.f[1][v][pc - (unsigned int)g.es[1]]; }
             if (g.act[2]) { fz1[v] = fx.f[2][v][pc]; fz0[v] = fx.f[2][v][pc - (unsigned int)g.es[2]]; }
-            ua5[v] = FORM == 3 ? 0.0 : Ua.q[v][oc];
-            ub5[v] = (FORM == 1 || FORM == 2) ? V.q[v][oc] : 0.0;           // U_(s) is the state the sweep ran on
+            ua5[v] = FORM == 3 ? 0.0 : ld_state<ST>(Ua.q[v], oc);
+            ub5[v] = (FORM == 1 || FORM == 2) ? ld_state<ST>(V.q[v], oc) : 0.0;           // U_(s) is the state the sweep ran on
         }
     }
 #pragma unroll
@@ -184,9 +190,14 @@ __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int li
             if (src.on && v < 2) L = L + S;
             const double ua = ua5[v], ub = ub5[v];
             W[v] = FORM == 0 ? ua + dt * L : (FORM == 1 ? 0.5 * (ua + ub + dt * L) : (FORM == 2 ? sg.ca * ua + sg.cb * ub + (sg.cdt * dt) * L : L));
-            out.q[v][oc] = W[v];
+            if (FORM == 3) out.q[v][oc] = W[v];                            // L itself (mf_eval_L): double whatever the state precision
+            else st_state<ST>(out.q[v], oc, W[v]);
         }
-        if (CFL) smax = signal_speed<0>(q, W[0], W[1], W[2], W[3], W[4], bad);
+        if (CFL) {                                                         // S_max of the STORED (rounded) new state
+#pragma unroll
+            for (int v = 0; v < 5; ++v) W[v] = as_stored<ST>(W[v]);
+            smax = signal_speed<0>(q, W[0], W[1], W[2], W[3], W[4], bad);
+        }
     }
     if (CFL) block_reduce_smax<XT>(smax, bad, ds);
 }
@@ -196,6 +207,7 @@ __global__ void __launch_bounds__(XT, XB) k_sweep_xcombine(Grid g, Eos q, int li
 bool sweep_supported(const Grid& g, int eos_kind, int predictor)
 {
     if (!g.act[0] || eos_kind != 0) return false;                             // the x sweep finishes the cells; closed-form EOS only
+    if (g.state32 && predictor) return false;                                 // k_delta_stage reads an fp64 state
     if (predictor && !(g.act[1] && g.act[2] && g.nev == 1)) return false;     // delta comes from k_delta_stage (3D, one event)
     return true;
 }
@@ -208,8 +220,11 @@ int launch_sweep_flux(const Grid& g, const Eos& q, int limiter, int k, bool pred
         long long total = 1;
         for (int a = 0; a < 3; ++a) total *= (a == d) ? g.n[a] + 1 : g.n[a];
         const dim3 nb((unsigned int)((total + TPB - 1) / TPB), g.nev);
-        if (d == 1) { if (pred) k_sweep_flux<1, true><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds); else k_sweep_flux<1, false><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds); }
-        else        { if (pred) k_sweep_flux<2, true><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds); else k_sweep_flux<2, false><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds); }
+#define MF_SF(D_, ST_) do { if (pred) k_sweep_flux<D_, true, ST_><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds); \
+                            else k_sweep_flux<D_, false, ST_><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds); } while (0)
+        if (d == 1) { if (g.state32) MF_SF(1, float); else MF_SF(1, double); }
+        else        { if (g.state32) MF_SF(2, float); else MF_SF(2, double); }
+#undef MF_SF
         ++launches;
     }
     return launches;
@@ -220,7 +235,8 @@ int launch_sweep_xcombine(const Grid& g, const Eos& q, int limiter, int k, bool 
 {
     const long long total = (long long)(g.n[0] + 1) * g.n[1] * g.n[2];
     const dim3 nb((unsigned int)((total + XT - 2) / (XT - 1)), g.nev);
-#define MF_SXC(P_, FORM_, CFL_) k_sweep_xcombine<P_, FORM_, CFL_><<<nb, XT, 0, st>>>(g, q, limiter, k, V, Dl, fx, sg, Ua, out, src, ds)
+#define MF_SXC(P_, FORM_, CFL_) do { if (g.state32) k_sweep_xcombine<P_, FORM_, CFL_, float><<<nb, XT, 0, st>>>(g, q, limiter, k, V, Dl, fx, sg, Ua, out, src, ds); \
+                                     else k_sweep_xcombine<P_, FORM_, CFL_, double><<<nb, XT, 0, st>>>(g, q, limiter, k, V, Dl, fx, sg, Ua, out, src, ds); } while (0)
 #define MF_SXC_FORMS(P_) \
     if (sg.form == 0) { if (sg.cfl) MF_SXC(P_, 0, true); else MF_SXC(P_, 0, false); } \
     else if (sg.form == 1) { if (sg.cfl) MF_SXC(P_, 1, true); else MF_SXC(P_, 1, false); } \
