@@ -159,6 +159,22 @@ def test_predictor_off_paths_agree_bit_for_bit_in_32_bit_state_mode(path):
     assert not all(np.array_equal(a, F32(a)) for a in L)
 
 
+def test_tabulated_eos_with_32_bit_state_strict():
+    """The two widening rows together: tabulated p(e, n) with Newton con2prim (reading A18) on a single-precision state (A19)."""
+    st = w.lumpy_event(shape=(9, 11, 13), dx=0.25, n_gauss=4, radius=0.8, half_z=0.6, background=0.5)
+    nz, ny, nx = st["shape"]
+    table = w.crossover_eos_table()
+    kw = dict(limiter="mc", k_stages=2, rk=3, bc="outflow")
+    g = MustaForce(nx, ny, nz, dx=st["dx"], strict=True, state_bits=32, eos_table=table, **kw)
+    o = Oracle(nx, ny, nz, dx=st["dx"], state_bits=32, eos_table=table, **kw)
+    for h in (g, o):
+        h.set_state(*[st[f] for f in FIELDS])
+        h.step(5, 0.3)
+    for a, b in zip(g.get_state(), o.get_state()):
+        assert np.all(np.isfinite(a)) and np.array_equal(a, F32(a))
+        assert np.abs(a - b.reshape(a.shape)).max() <= 1e-6 * np.abs(b).max()      # (log/exp of the table path are library calls: not bit-comparable)
+
+
 def test_batch_of_events_32_bit_state():
     evs = [w.lumpy_event(event=e, shape=(10, 12, 14), dx=0.2, n_gauss=4, radius=0.8, half_z=0.5, background=0.5) for e in range(3)]
     nz, ny, nx = evs[0]["shape"]
