@@ -105,19 +105,21 @@ State5 state(double* base, long long n) { State5 s; for (int v = 0; v < 5; ++v) 
 
 // Component pointers of a STATE REGISTER: nst elements per component of the context's state element type (double, or float in 32-bit state
 // mode, reading A19).  The structs carry double pointers either way; the kernels of the staged path cast them back (ld_state / st_state).
-CState5 creg(const mf_ctx* c, const double* base, long long first = 0)
+CState5 creg_as(const mf_ctx* c, const double* base, bool f32, long long first = 0)
 {
     CState5 s;
     for (int v = 0; v < 5; ++v)
-        s.q[v] = c->g.state32 ? reinterpret_cast<const double*>(reinterpret_cast<const float*>(base) + v * c->nst + first) : base + v * c->nst + first;
+        s.q[v] = f32 ? reinterpret_cast<const double*>(reinterpret_cast<const float*>(base) + v * c->nst + first) : base + v * c->nst + first;
     return s;
 }
-State5 reg(const mf_ctx* c, double* base)
+State5 reg_as(const mf_ctx* c, double* base, bool f32)
 {
     State5 s;
-    for (int v = 0; v < 5; ++v) s.q[v] = c->g.state32 ? reinterpret_cast<double*>(reinterpret_cast<float*>(base) + v * c->nst) : base + v * c->nst;
+    for (int v = 0; v < 5; ++v) s.q[v] = f32 ? reinterpret_cast<double*>(reinterpret_cast<float*>(base) + v * c->nst) : base + v * c->nst;
     return s;
 }
+CState5 creg(const mf_ctx* c, const double* base, long long first = 0) { return creg_as(c, base, c->g.state32 != 0, first); }
+State5 reg(const mf_ctx* c, double* base) { return reg_as(c, base, c->g.state32 != 0); }
 
 Faces faces_of(mf_ctx* c)
 {
@@ -1048,10 +1050,7 @@ int mf_set_state_precision(mf_ctx* c, int bits)
     }
     // the stored state changes its element type: U^n is converted into the next register (free between steps), which becomes U^n
     const int next = (c->cur + 1) % c->nreg;
-    c->g.state32 = keep;                                           // creg / reg describe the source in its present type ...
-    const CState5 src = creg(c, c->U[c->cur]);
-    c->g.state32 = on;                                             // ... and the destination in the new one
-    c->launches += launch_state_convert(c->nst, on, src, reg(c, c->U[next]), c->num_sms, c->stream);
+    c->launches += launch_state_convert(c->nst, on, creg_as(c, c->U[c->cur], keep != 0), reg_as(c, c->U[next], on != 0), c->num_sms, c->stream);
     c->cur = next;
     c->smax_valid = 0;                                             // S_max is taken from the stored (rounded) state
     int rc = check_launch(c);
