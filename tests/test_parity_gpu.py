@@ -240,13 +240,14 @@ def test_device_pointer_state_io_and_user_stream():
     assert g.launch_count() > 0
 
 
-def test_async_state_io_streams_events_through_several_contexts():
+@pytest.mark.parametrize("bits", [64, 32])
+def test_async_state_io_streams_events_through_several_contexts(bits):
     """mf_set_state_async / mf_get_state_async: three contexts on their own streams, events handed round-robin with pinned buffers; every
     event's result equals the synchronous calls' bit for bit, and the buffers are complete after mf_sync."""
     import torch
     events = [w.lumpy_event(event=e, shape=(12, 14, 16), dx=0.3) for e in range(7)]
     F = ("E", "Mx", "My", "Mz", "R")
-    ctxs = [MustaForce(16, 14, 12, dx=0.3, limiter="mc", k_stages=2, rk=3) for _ in range(3)]
+    ctxs = [MustaForce(16, 14, 12, dx=0.3, limiter="mc", k_stages=2, rk=3, state_bits=bits) for _ in range(3)]
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
     ins = [[pin(ev[f]) for f in F] for ev in events]
     outs = [[pin(np.zeros_like(ev["E"])) for _ in F] for ev in events]
@@ -258,7 +259,7 @@ def test_async_state_io_streams_events_through_several_contexts():
         c.get_state_async(outs[i])
     for c in ctxs:
         assert c.sync() == 0
-    ref = MustaForce(16, 14, 12, dx=0.3, limiter="mc", k_stages=2, rk=3)
+    ref = MustaForce(16, 14, 12, dx=0.3, limiter="mc", k_stages=2, rk=3, state_bits=bits)
     for i, ev in enumerate(events):
         ref.set_state(*[ev[f] for f in F])
         ref.step(4, 0.3)
