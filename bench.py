@@ -497,7 +497,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (default 3 = the 256^3 metric workload)")
     ap.add_argument("--grid", default=None, help="nz,ny,nx override (parity/debug sizes)")
-    ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid", "sweep"])
+    ap.add_argument("--path", default="auto", choices=["auto", "staged", "fused", "hybrid", "sweep", "small"])
     ap.add_argument("--eos", default="cs2", choices=["cs2", "table"], help="table: synthetic crossover p(e,n) table with Newton con2prim")
     ap.add_argument("--predictor", default="on", choices=["on", "off"], help="off: without the Hancock half step (reading A4), reported beside the default")
     ap.add_argument("--k", type=int, default=None, help="override the number of MUSTA stages (e.g. 4: the paper's own setting, PAPER.md:256)")

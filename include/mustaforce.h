@@ -55,7 +55,11 @@ enum { MF_PATH_AUTO = 0   /* fastest path that supports the configuration */,
        MF_PATH_SWEEP = 4  /* per-direction sweep kernels that limit the slopes themselves from a +-2-cell halo of the state (:33 "each dimension
                              separately"): no face states in HBM.  Needs an active x axis and MF_EOS_CS2; with the Hancock predictor on also a
                              3D grid and a single event (a predictor kernel then writes the increment of Eq.13 once per cell).  MF_PATH_AUTO
-                             takes it whenever the predictor is off. */ };
+                             takes it whenever the predictor is off. */,
+       MF_PATH_SMALL = 5  /* small 1D grids (nx <= 766, ny = nz = 1, MF_EOS_CS2, one event, fp64 state, three state registers): ONE launch of ONE
+                             block runs all n steps of an mf_step / mf_step_dt call - S_max and dt by a block reduction at the start of every
+                             step, the stages synchronised with __syncthreads, face data and fluxes in shared memory.  Same arithmetic as the
+                             staged path.  MF_PATH_AUTO takes it where it applies: such grids are launch bound on every other path. */ };
 
 /* Create a context for an nx*ny*nz grid of spacing dx (same on every axis).  An axis of extent 1 is inactive
  * (ny = nz = 1 is the 1D scheme); an active axis needs extent >= 4; the grid with its boundary layer must have fewer

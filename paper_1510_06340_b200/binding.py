@@ -15,7 +15,7 @@ MF_OK, MF_EINVAL, MF_ENOMEM, MF_ECUDA, MF_ESTATE = 0, -1, -2, -3, -4
 MF_EOS_CS2, MF_EOS_TABLE = 0, 1
 LIM = {"none": 0, "minmod": 1, "superbee": 2, "vanalbada": 3, "vanleer": 4, "mc": 5, "first": 6}
 BC = {"outflow": 0, "periodic": 1}
-PATH = {"auto": 0, "staged": 1, "fused": 2, "hybrid": 3, "sweep": 4}
+PATH = {"auto": 0, "staged": 1, "fused": 2, "hybrid": 3, "sweep": 4, "small": 5}
 
 _dp = C.POINTER(C.c_double)
 _vp = C.c_void_p

@@ -187,7 +187,12 @@ int resolve_path(mf_ctx* c)
         if (!sweep_supported(c->g, c->q.kind || c->eos != MF_EOS_CS2, c->predictor)) return MF_EINVAL;
         c->path = MF_PATH_SWEEP;
     }
+    else if (c->path_req == MF_PATH_SMALL) {
+        if (!small_supported(c->g, c->q.kind || c->eos != MF_EOS_CS2)) return MF_EINVAL;
+        c->path = MF_PATH_SMALL;
+    }
     else if (c->path_req == MF_PATH_STAGED) c->path = MF_PATH_STAGED;
+    else if (small_supported(c->g, c->q.kind || c->eos != MF_EOS_CS2)) c->path = MF_PATH_SMALL;      // AUTO: launch-bound grids
     else {
         // AUTO.  Predictor on: the staged path measured faster than the fused path on B200 (profiles/).  Predictor off: the sweep kernels
         // need no cell stage and no face-state scratch.
@@ -726,7 +731,7 @@ int mf_get_state_prim(mf_ctx* c, double* e, double* vx, double* vy, double* vz, 
 static int begin_step(mf_ctx* c, int mode, double value)
 {
     c->launches += launch_begin_step(c->ds, c->dsc, c->nev, mode, value, c->g.dx, c->alpha, c->stream);
-    if (c->g.cslot >= 0 && (c->path == MF_PATH_STAGED || c->path == MF_PATH_HYBRID)) {
+    if (c->g.cslot >= 0 && (c->path == MF_PATH_STAGED || c->path == MF_PATH_HYBRID || c->path == MF_PATH_SMALL)) {   // (SMALL: mf_eval_L runs staged kernels)
         if (upload_step_const_staged(c->dsc, c->g.cslot, c->nev, c->stream) != 0) { cudaGetLastError(); return fail(c, MF_ECUDA, "copy of the step scalars to constant memory failed"); }
     }
     if (c->g.cslot >= 0 && c->path == MF_PATH_HYBRID) {
@@ -756,6 +761,15 @@ static int enqueue_step(mf_ctx* c, int mode, double value)
 static int run_steps(mf_ctx* c, int n, int mode, double value)
 {
     int done = 0, rc;
+    if (c->path == MF_PATH_SMALL && n > 0) {
+        // the whole call is one launch: the kernel takes S_max of U^n itself at every step, rotates the registers like run_step and keeps the clock
+        int ps = prof_begin(c, 4);
+        c->launches += launch_small_steps(c->g, c->q, c->limiter, c->predictor, c->k, c->rk, c->alpha, mode, value, n, c->cur, c->U, c->src, c->ds, c->stream);
+        prof_end(c, ps);
+        c->cur = (c->cur + (long long)n * (c->rk == 2 ? 2 : 1)) % 3;
+        c->smax_valid = 0;
+        return check_launch(c);
+    }
     const int period = c->nreg;                                   // cur returns to its value after this many steps (RK2 and RK3 alike)
     if (c->graph_on && !c->prof_on && n >= 1 + 2 * period) {
         if ((rc = enqueue_step(c, mode, value)) != MF_OK) return rc;
@@ -1005,10 +1019,10 @@ int mf_set_path(mf_ctx* c, int path)
 {
     if (!c) return MF_EINVAL;
     c->epoch++;
-    if (path < MF_PATH_AUTO || path > MF_PATH_SWEEP) return fail(c, MF_EINVAL, "unknown path");
+    if (path < MF_PATH_AUTO || path > MF_PATH_SMALL) return fail(c, MF_EINVAL, "unknown path");
     int keep = c->path_req;
     c->path_req = path;
-    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "this path does not support this configuration (fused/hybrid: three active axes, MF_EOS_CS2, one event; sweep: active x axis, MF_EOS_CS2, and with the predictor on a 3D grid and one event; low storage: staged only)"); }
+    if (resolve_path(c) != MF_OK) { c->path_req = keep; resolve_path(c); return fail(c, MF_EINVAL, "this path does not support this configuration (fused/hybrid: three active axes, MF_EOS_CS2, one event; sweep: active x axis, MF_EOS_CS2, and with the predictor on a 3D grid and one event; small: 1D, nx <= 766, MF_EOS_CS2, one event; low storage: staged only)"); }
     return MF_OK;
 }
 int mf_set_low_storage(mf_ctx* c, int on)

@@ -55,6 +55,11 @@ int launch_tile_stage_pre(const Grid& g, const Eos& q, int k, Faces fc, CState5 
 int upload_step_const_tile(const StepConst* dsc, int slot, int nev, cudaStream_t st);   // the tile unit's constant-memory step scalars; 0 = ok
 bool tile_reduces_cfl();
 
+// ---- small 1D grids (MF_PATH_SMALL, mf_small.cu): all n steps of a call in ONE launch of ONE block (S_max, dt, RK stages, clock on the device)
+bool small_supported(const Grid& g, int eos_kind);
+int launch_small_steps(const Grid& g, const Eos& q, int limiter, int predictor, int k, int rk, double alpha, int mode, double value, int nsteps,
+                       int cur, double* const U[3], Source src, StepState* ds, cudaStream_t st);
+
 // ---- sweep path (MF_PATH_SWEEP, mf_sweep.cu): per-direction sweeps that limit the slopes themselves from a +-2-cell halo of V; with pred the
 // Hancock increment Dl (extended layout, from launch_delta_stage) is added to both face states.  F_y, F_z go to fx, the x sweep finishes the cells.
 bool sweep_supported(const Grid& g, int eos_kind, int predictor);

@@ -13,7 +13,7 @@ from paper_1510_06340_b200.binding import MustaForce, MustaForceError, MF_ESTATE
 
 pytestmark = pytest.mark.gpu
 
-PATHS = ["staged", "fused", "hybrid", "sweep"]
+PATHS = ["staged", "fused", "hybrid", "sweep", "small"]
 
 
 def _skip_unsupported(fn):
