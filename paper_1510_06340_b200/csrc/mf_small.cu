@@ -99,7 +99,9 @@ __device__ __forceinline__ void small_cell_rt(int lim, const Grid& g, const Eos&
     }
 }
 
-__global__ void __launch_bounds__(768, 1)
+// MAXT: the largest block this instantiation is launched with (512: up to 128 registers per thread, no spills; 768: 80)
+template <int MAXT>
+__global__ void __launch_bounds__(MAXT, 1)
 k_small1d(Grid g, Eos q, SmallArgs a, double* U0p, double* U1p, double* U2p, Source src, StepState* ds)
 {
     extern __shared__ double sm[];                       // [n+2][5] lo, [n+2][5] hi, [n+1][5] F
@@ -220,8 +222,12 @@ int launch_small_steps(const Grid& g, const Eos& q, int limiter, int predictor, 
     const int threads = ((n + 2 + 31) / 32) * 32;
     const size_t smem = sizeof(double) * (size_t)(15 * (n + 2));
     static DeviceOnce once;
-    if (once.first()) cudaFuncSetAttribute(k_small1d, cudaFuncAttributeMaxDynamicSharedMemorySize, 15 * 768 * (int)sizeof(double));
-    k_small1d<<<1, threads, smem, st>>>(g, q, a, U[0], U[1], U[2], src, ds);
+    if (once.first()) {
+        cudaFuncSetAttribute(k_small1d<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, 15 * 512 * (int)sizeof(double));
+        cudaFuncSetAttribute(k_small1d<768>, cudaFuncAttributeMaxDynamicSharedMemorySize, 15 * 768 * (int)sizeof(double));
+    }
+    if (threads <= 512) k_small1d<512><<<1, threads, smem, st>>>(g, q, a, U[0], U[1], U[2], src, ds);
+    else k_small1d<768><<<1, threads, smem, st>>>(g, q, a, U[0], U[1], U[2], src, ds);
     return 1;
 }
 
