@@ -37,7 +37,7 @@ def test_predictor_off_takes_the_sweep_path_and_matches_the_oracle(index):
     """The five configs' schemes without the Hancock step, 100 steps at parity sizes, path chosen by MF_PATH_AUTO."""
     st = _scaled(index)
     g, o = parity.make_pair(st, predictor=False)
-    assert g.path() == "sweep"
+    assert g.path() == ("small" if index == 1 else "sweep")               # (config 1 is a launch-bound 1D grid: MF_PATH_AUTO runs it in one block)
     g.step(100, st["cfl"])
     o.step(100, st["cfl"])
     got, ref = g.get_state(), o.get_state()
@@ -119,6 +119,13 @@ def test_path_selection_rules():
     assert g.path() == "sweep"
     g = MustaForce(16, 16, 16, dx=0.1, predictor=False, eos_table=w.crossover_eos_table())
     assert g.path() == "staged"                                           # tabulated EOS: staged path only
+    # launch-bound 1D grids: MF_PATH_AUTO runs them in one block, whatever the predictor setting; larger ones and other options do not qualify
+    assert MustaForce(400, dx=0.1).path() == "small" and MustaForce(400, dx=0.1, predictor=False).path() == "small"
+    assert MustaForce(767, dx=0.1).path() == "staged" and MustaForce(767, dx=0.1, predictor=False).path() == "sweep"
+    assert MustaForce(400, dx=0.1, state_bits=32).path() == "staged"
+    assert MustaForce(400, dx=0.1, eos_table=w.crossover_eos_table()).path() == "staged"
+    with pytest.raises(MustaForceError):
+        MustaForce(16, 16, 1, dx=0.1, path="small")
 
 
 def test_sweep_conserves_and_keeps_a_uniform_state():
