@@ -2,7 +2,7 @@
  * mustaforce.h — C ABI of libmustaforce.so: the per-timestep MUSTA-FORCE update of ideal relativistic
  * hydrodynamics (arXiv 1510.06340) on a 3D Cartesian grid, fp64, hand-written CUDA for sm_100a.
  *
- * What one step computes (citations are PAPER.md lines; readings A1..A17 are listed in DESIGN.md):
+ * What one step computes (citations are PAPER.md lines; readings A1..A19 are listed in DESIGN.md):
  *   conservation system  dU/dt + dF/dx + dG/dy + dH/dz = 0,  U = (E, Mx, My, Mz, R)      Eq.1  :41-49
  *   fluxes               F_d = ((E+p)v_d, M_j v_d + p delta_jd, R v_d)                   Eq.3  :53-59
  *   con2prim             v = M/(E+p(e,n)), e = E - M.v, n = R sqrt(1-v^2)                Eq.23 :221-236

@@ -1,6 +1,6 @@
 // mf_device.cuh — per-cell / per-interface device arithmetic of the MUSTA-FORCE step (fp64, sm_100a).
 // Everything here lives in registers; the kernels in mf_kernels.cu decide where operands come from.
-// Citations are PAPER.md lines; readings A1..A17 are listed in DESIGN.md.
+// Citations are PAPER.md lines; readings A1..A19 are listed in DESIGN.md.
 #pragma once
 #include <cuda_runtime.h>
 
