@@ -25,7 +25,11 @@
  * the MUSTA_k predictor-corrector update Eq.8 against its closed form in k for a linear flux (a geometric
  * sequence; tests/test_oracle_pieces.py::test_musta_linear_flux_closed_form), the signal speed at rest / at
  * |v| -> 1 / as a sum of rapidities, and the source's RK stage times as the nodes of the trapezoidal and
- * Simpson rules on a one-cell grid (error orders dt^3, dt^5 against the exact erf integral).
+ * Simpson rules on a one-cell grid (error orders dt^3, dt^5 against the exact erf integral), and the MUSCL-Hancock
+ * half step with its face values (Eq.12-14, reading A3: ONE increment for all faces of a cell) through FORCE against the
+ * closed form of L for linear advection of the charge in 1D, 2D and 3D
+ * (tests/test_oracle_pieces.py::test_muscl_hancock_force_closed_form_for_linear_advection: a half-step factor of lam instead of
+ * lam/2, or its sign flipped, fails it).
  * Single-precision state mode (mfo_set_state_precision, reading A19): tests/test_oracle_state32.py - stored values are
  * floats, one step equals Eq.6 / Eq.7 composed in numpy with float32 rounding of every stage around the 64-bit mfo_eval_L, uniform
  * state fixed, conservation and distance to the 64-bit run at single-precision round-off.

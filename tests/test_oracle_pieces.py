@@ -192,6 +192,50 @@ def test_first_order_force_linear_stencil(alpha):
         assert np.all(np.abs(L[q]) < 1e-14)
 
 
+# ---------------------------------------------------------------- MUSCL-Hancock + FORCE on linear advection (pins Eq.12, Eq.13 and reading A3)
+@pytest.mark.parametrize("shape,v", [((1, 1, 32), (0.4, 0.0, 0.0)), ((7, 5, 6), (0.3, -0.2, 0.25)), ((1, 9, 8), (-0.35, 0.3, 0.0))])
+def test_muscl_hancock_force_closed_form_for_linear_advection(shape, v):
+    """With uniform (e, v) the charge R is advected linearly, flux_d = v_d R, and every step of the reconstruction is linear for the central
+    slope (Eq.14), so one evaluation of L has a closed form.  Written out here from the paper, not from the oracle:
+      slopes       s_d = (u_{+d} - u_{-d})/2                                             Eq.12, Eq.14
+      half step    delta = sum_d (lambda/2)(v_d u^{dL} - v_d u^{dR}) = -(1/2) sum_d c_d s_d,  c_d = v_d dt/dx
+                   - ONE increment for all faces of the cell (reading A3)                Eq.13  :165-171
+      faces        A_d = u + s_d/2 + delta (right face of the cell),  B_d = u_{+d} - s_d(+d)/2 + delta(+d)   :173
+      FORCE, k=0   lambda F_d = (c_d/2)(A_d + B_d) - (1/4)(alpha c_d^2 + 1/alpha)(B_d - A_d)   Eq.9-11  :139-149
+      L            = -(1/dt) sum_d (lambda F_d - lambda F_d(-d))                          Eq.1  :43
+    A wrong factor or sign in the half step, an increment added to one face only, or a per-direction increment all change the result."""
+    nz, ny, nx = shape
+    dx, dt = 0.5, 0.15
+    act = [nx > 1, ny > 1, nz > 1]
+    alpha = float(sum(act))
+    o = Oracle(nx, ny, nz, dx=dx, limiter="none", k_stages=0, predictor=True, bc="periodic")
+    rng = np.random.default_rng(11)
+    n = 1.0 + rng.uniform(size=shape)
+    full = lambda c: np.full(shape, c)
+    o.set_state_prim(full(2.0), full(v[0]), full(v[1]), full(v[2]), n)
+    u = o.get_state()[4]
+    L = o.eval_L(dt)
+    axes = {0: 2, 1: 1, 2: 0}                                            # direction d lives on numpy axis axes[d] of (nz, ny, nx)
+    plus = lambda a, d: np.roll(a, -1, axis=axes[d])
+    minus = lambda a, d: np.roll(a, 1, axis=axes[d])
+    c = [v[d] * dt / dx for d in range(3)]
+    s = {d: 0.5 * (plus(u, d) - minus(u, d)) for d in range(3) if act[d]}
+    delta = sum(-0.5 * c[d] * s[d] for d in s)
+    want = np.zeros(shape)
+    for d in s:
+        A = u + 0.5 * s[d] + delta
+        B = plus(u - 0.5 * s[d] + delta, d)
+        lamF = 0.5 * c[d] * (A + B) - 0.25 * (alpha * c[d] ** 2 + 1.0 / alpha) * (B - A)
+        want -= (lamF - minus(lamF, d)) / dt
+    assert np.allclose(L[4], want, rtol=0, atol=2e-13 * np.abs(want).max())
+    for q in range(4):                                                   # uniform E, M: nothing moves
+        assert np.all(np.abs(L[q]) < 1e-13)
+    # and the half step matters at the level this pin resolves: without it L differs by far more than the tolerance
+    o2 = Oracle(nx, ny, nz, dx=dx, limiter="none", k_stages=0, predictor=False, bc="periodic")
+    o2.set_state_prim(full(2.0), full(v[0]), full(v[1]), full(v[2]), n)
+    assert np.abs(o2.eval_L(dt)[4] - want).max() > 1e-3 * np.abs(want).max()
+
+
 def test_musta_flux_of_equal_states_is_the_physical_flux(orc):
     """Consistency: U_L = U_R = U gives F = F(U) for any k (Eq.8-11 reduce to the identity)."""
     U = orc.prim2con([2.0, 0.3, -0.2, 0.5, 1.5])
