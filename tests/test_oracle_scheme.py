@@ -351,6 +351,40 @@ def test_advection_in_3d_along_the_diagonal_converges():
 
 
 # ---------------------------------------------------------------- OpenMP build is the same oracle
+@pytest.mark.parametrize("rk", [2, 3])
+@pytest.mark.parametrize("k,predictor", [(0, False), (2, True)])
+def test_runge_kutta_step_is_the_taylor_polynomial_of_a_linear_operator(rk, k, predictor):
+    """Eq.6 / Eq.7 against what the mathematics fixes: for a LINEAR spatial operator the TVD RK2 step is
+    (1 + z + z^2/2) U and the TVD RK3 step (1 + z + z^2/2 + z^3/6) U with z = dt L (their stability polynomials).  L is linear in the charge R
+    when (e, v) are uniform (R is advected, flux v_d R) and the slope is the central one (Eq.14), whatever k and the half step do; powers of L
+    are taken with mfo_eval_L on states whose R is the previous result.  A wrong coefficient anywhere in Eq.6 or Eq.7 changes the polynomial."""
+    shape = (5, 6, 8)
+    nz, ny, nx = shape
+    dx, dt = 0.5, 0.12
+    v = (0.3, -0.2, 0.25)
+    full = lambda c: np.full(shape, c)
+    rng = np.random.default_rng(3)
+    kw = dict(dx=dx, limiter="none", k_stages=k, predictor=predictor, bc="periodic", rk=rk)
+    o = Oracle(nx, ny, nz, **kw)
+    o.set_state_prim(full(2.0), full(v[0]), full(v[1]), full(v[2]), 1.0 + rng.uniform(size=shape))
+    E, Mx, My, Mz, R0 = o.get_state()
+
+    def L(R):                                                             # the oracle's own spatial operator on (E, M, R)
+        h = Oracle(nx, ny, nz, **kw)
+        h.set_state(E, Mx, My, Mz, R)
+        out = h.eval_L(dt)
+        assert all(np.abs(out[q]).max() < 1e-13 for q in range(4))       # uniform E, M: nothing moves, so L acts on R alone
+        return out[4]
+
+    L1 = L(R0); L2 = L(L1); L3 = L(L2)
+    assert np.allclose(L(2.0 * R0 - 0.5 * L1), 2.0 * L1 - 0.5 * L2, rtol=0, atol=1e-12 * np.abs(L1).max())    # L is linear indeed
+    want = R0 + dt * L1 + 0.5 * dt ** 2 * L2 + ((dt ** 3 / 6.0) * L3 if rk == 3 else 0.0)
+    o.step_dt(1, dt)
+    got = o.get_state()[4]
+    assert np.allclose(got, want, rtol=0, atol=1e-13 * np.abs(want).max())
+    assert np.abs(got - (want + (dt ** 3 / 6.0) * L3 * (1 if rk == 2 else -1))).max() > 1e-8          # (and the orders differ measurably)
+
+
 def test_openmp_build_is_bit_identical():
     st = workloads.lumpy_event(shape=(10, 9, 12), dx=0.3, n_gauss=6, radius=1.2, half_z=1.0)
     out = []
