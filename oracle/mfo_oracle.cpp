@@ -31,6 +31,7 @@
  * (tests/test_oracle_pieces.py::test_muscl_hancock_force_closed_form_for_linear_advection: a half-step factor of lam instead of
  * lam/2, or its sign flipped, fails it), and the Runge-Kutta steps Eq.6 / Eq.7 against their stability polynomials 1 + z + z^2/2 (+ z^3/6)
  * for the linear operator of charge advection (tests/test_oracle_scheme.py::test_runge_kutta_step_is_the_taylor_polynomial_of_a_linear_operator).
+ * Ghost cells (reading A11): cyclic translation invariance on a periodic box (bit for bit) and mirror symmetry under outflow, per axis.
  * Single-precision state mode (mfo_set_state_precision, reading A19): tests/test_oracle_state32.py - stored values are
  * floats, one step equals Eq.6 / Eq.7 composed in numpy with float32 rounding of every stage around the 64-bit mfo_eval_L, uniform
  * state fixed, conservation and distance to the 64-bit run at single-precision round-off.

@@ -385,6 +385,48 @@ def test_runge_kutta_step_is_the_taylor_polynomial_of_a_linear_operator(rk, k, p
     assert np.abs(got - (want + (dt ** 3 / 6.0) * L3 * (1 if rk == 2 else -1))).max() > 1e-8          # (and the orders differ measurably)
 
 
+@pytest.mark.parametrize("shift", [(3, 0, 0), (0, -2, 0), (0, 0, 5), (1, 2, -3)])
+def test_periodic_box_is_translation_invariant(shift):
+    """Ghost cells of a periodic box are the cells modulo n on every axis (reading A11): shifting the initial data cyclically shifts the result,
+    bit for bit (every cell runs the same arithmetic on the same numbers).  A wrap that is off by one on any side of any axis breaks it."""
+    st = workloads.lumpy_event(shape=(7, 6, 9), dx=0.2, n_gauss=5, radius=0.6, half_z=0.4, background=0.5)
+    nz, ny, nx = st["shape"]
+    kw = dict(dx=st["dx"], limiter="mc", k_stages=2, rk=3, bc="periodic")
+    F = ("E", "Mx", "My", "Mz", "R")
+    a, b = Oracle(nx, ny, nz, **kw), Oracle(nx, ny, nz, **kw)
+    roll = lambda x: np.roll(x, shift, axis=(0, 1, 2))                   # shift = (z, y, x)
+    a.set_state(*[st[f] for f in F])
+    b.set_state(*[np.ascontiguousarray(roll(st[f])) for f in F])
+    a.step_dt(6, 0.02)
+    b.step_dt(6, 0.02)
+    for x, y in zip(a.get_state(), b.get_state()):
+        assert np.array_equal(roll(x), y)
+    assert not np.array_equal(a.get_state()[0], st["E"])
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_outflow_boundaries_are_mirror_symmetric(axis):
+    """Outflow ghosts are the clamped index on both sides of every axis (A11): data that are mirror symmetric about the middle of an axis stay so,
+    with the momentum component along that axis antisymmetric.  A clamp that treats the two ends differently breaks it."""
+    st = workloads.lumpy_event(shape=(8, 6, 10), dx=0.2, n_gauss=5, radius=0.5, half_z=0.4, background=0.5)
+    nz, ny, nx = st["shape"]
+    npax = {0: 2, 1: 1, 2: 0}[axis]                                       # direction -> numpy axis of (nz, ny, nx)
+    sym = lambda x: 0.5 * (x + np.flip(x, axis=npax))
+    e = sym(st["E"])
+    o = Oracle(nx, ny, nz, dx=st["dx"], limiter="superbee", k_stages=3, rk=3, bc="outflow")
+    zero = np.zeros_like(e)
+    o.set_state(e, zero, zero, zero, sym(st["R"]))
+    o.step(12, 0.3)
+    out = o.get_state()
+    scale = np.abs(out[0]).max()
+    for q, x in enumerate(out):
+        sign = -1.0 if q == 1 + axis else 1.0
+        assert np.abs(x - sign * np.flip(x, axis=npax)).max() <= 1e-13 * scale
+    assert np.abs(out[1 + axis]).max() > 1e-3 * scale                    # something moved, and it reached the boundary cells
+    edge = np.take(out[1 + axis], [0], axis=npax)
+    assert np.abs(edge).max() > 0.0
+
+
 def test_openmp_build_is_bit_identical():
     st = workloads.lumpy_event(shape=(10, 9, 12), dx=0.3, n_gauss=6, radius=1.2, half_z=1.0)
     out = []
