@@ -323,6 +323,52 @@ def test_full_size_config3_256_windows():
         print("256^3 window", centre, r)
 
 
+def test_full_size_config3_256_is_translation_invariant():
+    """A property that holds at any size (periodic box, reading A11), on the metric's workload in the launch configuration bench.py times:
+    shifting the initial state cyclically by (5, 3, 7) cells shifts the state after 10 steps, BIT FOR BIT - every cell runs the same
+    arithmetic on the same numbers wherever it sits in a block, a row or a plane, and S_max (hence every dt) is the same."""
+    st = w.gaussian_hot_spot()
+    nz, ny, nx = st["shape"]
+    assert (nz, ny, nx) == (256, 256, 256)
+    shift = (5, 3, 7)                                                     # (z, y, x)
+    outs = []
+    for sh in (None, shift):
+        g = MustaForce(nx, ny, nz, dx=st["dx"], **st["scheme"])
+        f = [st[k] if sh is None else np.ascontiguousarray(np.roll(st[k], sh, axis=(0, 1, 2))) for k in ("E", "Mx", "My", "Mz", "R")]
+        g.set_state(*f)
+        g.step(10, st["cfl"])
+        outs.append((g.get_state(), g.time()))
+        assert g.path() == "staged" and g.last_status == 0
+        g.close()
+    assert outs[0][1] == outs[1][1]
+    for a, b in zip(outs[0][0], outs[1][0]):
+        assert np.array_equal(np.roll(a, shift, axis=(0, 1, 2)), b)
+    assert np.abs(outs[0][0][1]).max() > 0.0
+
+
+def test_full_size_512_outflow_is_mirror_symmetric():
+    """The same kind of property for the outflow boundary at config 5's size and scheme (512^3, MC, k=3, RK3): a state that is mirror symmetric
+    about the middle of every axis stays so, with the momentum along an axis antisymmetric - the clamp treats both ends of every axis alike,
+    at the grid size where the unsigned 32-bit cell offsets are largest."""
+    n = 512
+    st = w.gaussian_hot_spot(n=n, dx=0.04, width=3.0)                     # wide enough to reach the faces within a few steps
+    g = MustaForce(n, n, n, dx=st["dx"], limiter="mc", k_stages=3, rk=3, bc="outflow")
+    g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+    g.step(4, 0.3)
+    out = g.get_state()
+    assert g.last_status == 0
+    g.close()
+    scale = float(np.abs(out[0]).max())
+    for axis, npax in ((0, 2), (1, 1), (2, 0)):
+        for q, x in enumerate(out):
+            sign = -1.0 if q == 1 + axis else 1.0
+            half = n // 2
+            lo = np.take(x, range(half), axis=npax)
+            hi = np.flip(np.take(x, range(half, n), axis=npax), axis=npax)
+            assert np.abs(lo - sign * hi).max() <= 1e-13 * scale
+    assert np.abs(np.take(out[1], [0], axis=2)).max() > 0.0               # the flow has reached the boundary cells
+
+
 def test_full_size_config2_128_window():
     st = w.diagonal_shock_3d()
     r = _windowed_parity(st, (64, 64, 64))                           # the shock front and the rarefaction pass through the centre
