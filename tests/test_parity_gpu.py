@@ -97,6 +97,26 @@ def test_config1_to_t12_matches_oracle_and_exact_solution(path):
     assert st["dx"] * np.abs(n - ne).sum() <= 2.4
 
 
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("shape", [(9, 11, 13), (1, 1, 37)])
+def test_other_sound_speed_and_force_alpha(shape, path):
+    """mf_set_cs2 and mf_set_alpha (p = cs2 e with cs2 != 1/3; FORCE-alpha with alpha != number of axes, :151): the strict
+    build bit for bit, the product build at the 1e-11 bar after 60 steps, S_max (which carries cs) included."""
+    st = w.lumpy_event(shape=shape, dx=0.25, n_gauss=4, radius=0.8, half_z=0.6, background=0.5)
+    kw = dict(limiter="mc", k_stages=2, rk=3, bc="periodic", cs2=0.2, alpha=1.7)
+    for strict in (True, False):
+        g, o = _skip_unsupported(lambda: parity.make_pair(st, path=path, strict=strict, **kw))
+        g.step(60, 0.3)
+        o.step(60, 0.3)
+        got, ref = g.get_state(), o.get_state()
+        assert g.last_status == 0 and o.status() == 0
+        if strict:
+            assert all(np.array_equal(a, b.reshape(a.shape)) for a, b in zip(got, ref)) and g.time() == o.time()
+        else:
+            parity.assert_parity(got, ref, what="cs2 = 0.2, alpha = 1.7 (%s)" % path)
+            assert g.max_signal_speed()[0] == pytest.approx(o.max_signal_speed()[0], rel=1e-13)
+
+
 # ------------------------------------------------------------------ strict build: bit-for-bit
 CASES = [("minmod", 2, 2, "outflow", True), ("superbee", 3, 3, "periodic", True), ("mc", 2, 2, "outflow", True),
          ("vanleer", 1, 3, "periodic", False), ("vanalbada", 4, 3, "outflow", True), ("none", 0, 2, "periodic", True),
