@@ -289,6 +289,32 @@ def test_async_state_io_streams_events_through_several_contexts(bits):
         ctxs[0].set_state_async(*[x.astype(np.float32) for x in ins[0]])
 
 
+def test_profile_classes_and_launch_count():
+    """mf_profile / mf_profile_read (what bench.py's roofline objects are timed with) and mf_launch_count: per RK stage one cell-stage group,
+    one flux group and one combine group on the staged path; recording changes no result; the counts match the launches."""
+    st = w.gaussian_hot_spot(shape=(20, 24, 28), dx=0.3)
+    nz, ny, nx = st["shape"]
+    a = MustaForce(nx, ny, nz, dx=st["dx"], **st["scheme"])
+    b = MustaForce(nx, ny, nz, dx=st["dx"], **st["scheme"])
+    for g in (a, b):
+        g.set_state(st["E"], st["Mx"], st["My"], st["Mz"], st["R"])
+    a.step(1, 0.3)
+    b.step(1, 0.3)
+    l0 = a.launch_count()
+    a.profile(True)
+    a.step(4, 0.3)
+    a.profile(False)
+    prof = a.profile_read()
+    b.step(4, 0.3)
+    assert a.path() == "staged"
+    assert {k: v[1] for k, v in prof.items()} == {"cell_stage": 12, "flux_stage": 12, "combine": 12}       # 4 steps x 3 RK stages
+    assert all(v[0] > 0.0 for v in prof.values())
+    assert a.launch_count() - l0 == 4 * (3 * 3 + 2)                       # + k_begin_step and k_end_step per step (y and z interfaces: one launch)
+    assert a.profile_read() == {}                                         # a read clears
+    for x, y in zip(a.get_state(), b.get_state()):
+        assert np.array_equal(x, y)
+
+
 # ------------------------------------------------------------------ full-size grids: windowed parity (DESIGN.md "Parity at full size")
 def _windowed_parity(st, centre, steps_before=95, m=5, half=8, path="auto"):
     """Advance the FULL grid on the GPU to step steps_before, then re-run the last m steps with the oracle on a sub-box around `centre`
