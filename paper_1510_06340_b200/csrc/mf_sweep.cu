@@ -65,12 +65,13 @@ __device__ __forceinline__ void halo4(int c, int n, int periodic, unsigned int s
 // =========================================================================== a1 + a3 + a5 + a6 along y or z
 // One thread per interface between cells c and c+e_D; c runs over -1..n_D-1 along D and the interior on the other axes.
 template <int D, bool PRED, class ST>
-__global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, int k, CState5 V, CState5 Dl, Fluxes fx, const StepState* ds)
+__device__ __forceinline__ void sweep_flux_body(const Grid& g, const Eos& q, int lim, int k, const CState5& V, const CState5& Dl, const Fluxes& fx,
+                                                const StepState* ds, unsigned int block)
 {
     int m[3] = { g.n[0], g.n[1], g.n[2] };
     m[D] += 1;
     const long long total = (long long)m[0] * m[1] * m[2];
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long t = (long long)block * blockDim.x + threadIdx.x;
     if (t >= total) return;
     int c[3];
     unflatten3((unsigned int)t, g.dv[0][D == 0], g.dv[1][D == 1], c[0], c[1], c[2]);
@@ -101,6 +102,20 @@ __global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, i
     musta_flux<D, 0>(q, k, musta_coef_of(ds), A, B, F);
 #pragma unroll
     for (int v = 0; v < 5; ++v) fx.f[D][v][p] = F[v];
+}
+
+template <int D, bool PRED, class ST>
+__global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, int k, CState5 V, CState5 Dl, Fluxes fx, const StepState* ds)
+{
+    sweep_flux_body<D, PRED, ST>(g, q, lim, k, V, Dl, fx, ds, blockIdx.x);
+}
+
+// the y and the z sweep of a stage are independent: one launch for both (blocks [0, nby) take y, the rest z), one kernel boundary less
+template <bool PRED, class ST>
+__global__ void __launch_bounds__(TPB, 3) k_sweep_flux_yz(Grid g, Eos q, int lim, int k, CState5 V, CState5 Dl, Fluxes fx, const StepState* ds, unsigned int nby)
+{
+    if (blockIdx.x < nby) sweep_flux_body<1, PRED, ST>(g, q, lim, k, V, Dl, fx, ds, blockIdx.x);
+    else sweep_flux_body<2, PRED, ST>(g, q, lim, k, V, Dl, fx, ds, blockIdx.x - nby);
 }
 
 // =========================================================================== a1 + a3 + a5 (x) + a6 + a7 + a8 (+ a2)
@@ -215,6 +230,16 @@ bool sweep_supported(const Grid& g, int eos_kind, int predictor)
 int launch_sweep_flux(const Grid& g, const Eos& q, int limiter, int k, bool pred, CState5 V, CState5 Dl, Fluxes fx, const StepState* ds, cudaStream_t st)
 {
     int launches = 0;
+    if (g.act[1] && g.act[2]) {
+        const unsigned int nby = (unsigned int)(((long long)g.n[0] * (g.n[1] + 1) * g.n[2] + TPB - 1) / TPB);
+        const unsigned int nbz = (unsigned int)(((long long)g.n[0] * g.n[1] * (g.n[2] + 1) + TPB - 1) / TPB);
+        const dim3 nb(nby + nbz, g.nev);
+#define MF_SFYZ(ST_) do { if (pred) k_sweep_flux_yz<true, ST_><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds, nby); \
+                          else k_sweep_flux_yz<false, ST_><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds, nby); } while (0)
+        if (g.state32) MF_SFYZ(float); else MF_SFYZ(double);
+#undef MF_SFYZ
+        return 1;
+    }
     for (int d = 1; d < 3; ++d) {
         if (!g.act[d]) continue;
         long long total = 1;
