@@ -110,7 +110,7 @@ def alg_bytes(rk, state_bytes=8):
 # --set full captures committed under profiles/ - measured once under ncu, not during this run: the JSON line names the file
 # ("traffic_source"), and nothing is reported for a workload, path or state precision without a committed capture.
 NCU_TRAFFIC_256 = {
-    ("staged", True): ("profiles/r02_ncu_full_staged_256.md", {"cell_stage": 3.396, "flux_stage": 4.091, "combine": 4.716}),
+    ("staged", True): ("profiles/r02_ncu_full_staged_256.md", {"cell_stage": 3.396, "flux_stage": 3.409, "combine": 4.716}),
     ("hybrid", True): ("profiles/r02_ncu_hybrid_tile3_256.md", {"fused_stage": 5.602}),
     ("sweep", False): ("profiles/r01_ncu_full_sweep_256.md", {"flux_stage": 2.664, "combine": 3.359}),
 }

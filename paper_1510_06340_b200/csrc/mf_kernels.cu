@@ -24,6 +24,9 @@ namespace mf {
 #ifndef MF_CELL_PF
 #define MF_CELL_PF (148 * 768)   // cells ahead (in the plane above) whose lines a cell-stage thread prefetches to L2: one wave of resident threads; 0 = off
 #endif
+#ifndef MF_YZ_INTERLEAVE
+#define MF_YZ_INTERLEAVE 1       // y and z flux blocks alternate in the merged launch (W is read from HBM once for both)
+#endif
 #ifndef MF_CELL_MINB
 #define MF_CELL_MINB (768 / MF_CELL_TPB)
 #endif
@@ -334,8 +337,16 @@ __global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage(Grid g, Eos q, 
 template <int EK, bool UC>
 __global__ void __launch_bounds__(FT, MF_FLUX_MINB) k_flux_stage_yz(Grid g, Eos q, int k, CState5 Wc, Faces fc, Fluxes fx, const StepState* ds, unsigned int nby)
 {
+#if MF_YZ_INTERLEAVE
+    // even blocks take y, odd blocks z, of the same stretch of cells: the W lines a y block reads are read again by the z block next to it
+    // while they are still in L2 (W(k) is the y block's plane and the z block's upper plane), so W crosses HBM once for the two directions
+    const unsigned int b = blockIdx.x >> 1;
+    if ((blockIdx.x & 1u) == 0) { if (b < nby) flux_stage_body<1, EK, UC>(g, q, k, Wc, fc, fx, ds, b); }
+    else flux_stage_body<2, EK, UC>(g, q, k, Wc, fc, fx, ds, b);
+#else
     if (blockIdx.x < nby) flux_stage_body<1, EK, UC>(g, q, k, Wc, fc, fx, ds, blockIdx.x);
     else flux_stage_body<2, EK, UC>(g, q, k, Wc, fc, fx, ds, blockIdx.x - nby);
+#endif
 }
 
 int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, Fluxes fx, const StepState* ds, cudaStream_t st)
@@ -346,7 +357,11 @@ int launch_flux_stage(const Grid& g, const Eos& q, int k, int dmask, Faces fc, F
 #ifndef MF_NO_YZ_MERGE
     if (dmask == 6 && g.act[1] && g.act[2]) {
         const unsigned int nby = blocks_for((long long)g.n[0] * (g.n[1] + 1) * g.n[2], FT), nbz = blocks_for((long long)g.n[0] * g.n[1] * (g.n[2] + 1), FT);
+#if MF_YZ_INTERLEAVE
+        const dim3 nb(2 * (nby > nbz ? nby : nbz), g.nev);
+#else
         const dim3 nb(nby + nbz, g.nev);
+#endif
         if (q.kind) k_flux_stage_yz<1, false><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds, nby);
         else if (g.cslot >= 0) k_flux_stage_yz<0, true><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds, nby);
         else k_flux_stage_yz<0, false><<<nb, FT, 0, st>>>(g, q, k, Wc, fc, fx, ds, nby);
