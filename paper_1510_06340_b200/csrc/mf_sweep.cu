@@ -110,12 +110,14 @@ __global__ void __launch_bounds__(TPB, 3) k_sweep_flux(Grid g, Eos q, int lim, i
     sweep_flux_body<D, PRED, ST>(g, q, lim, k, V, Dl, fx, ds, blockIdx.x);
 }
 
-// the y and the z sweep of a stage are independent: one launch for both (blocks [0, nby) take y, the rest z), one kernel boundary less
+// the y and the z sweep of a stage are independent: one launch for both, one kernel boundary less
 template <bool PRED, class ST>
 __global__ void __launch_bounds__(TPB, 3) k_sweep_flux_yz(Grid g, Eos q, int lim, int k, CState5 V, CState5 Dl, Fluxes fx, const StepState* ds, unsigned int nby)
 {
-    if (blockIdx.x < nby) sweep_flux_body<1, PRED, ST>(g, q, lim, k, V, Dl, fx, ds, blockIdx.x);
-    else sweep_flux_body<2, PRED, ST>(g, q, lim, k, V, Dl, fx, ds, blockIdx.x - nby);
+    // even blocks take y, odd blocks z of the same stretch of cells (the lines one reads are still in L2 when the other reads them)
+    const unsigned int b = blockIdx.x >> 1;
+    if ((blockIdx.x & 1u) == 0) { if (b < nby) sweep_flux_body<1, PRED, ST>(g, q, lim, k, V, Dl, fx, ds, b); }
+    else sweep_flux_body<2, PRED, ST>(g, q, lim, k, V, Dl, fx, ds, b);
 }
 
 // =========================================================================== a1 + a3 + a5 (x) + a6 + a7 + a8 (+ a2)
@@ -233,7 +235,7 @@ int launch_sweep_flux(const Grid& g, const Eos& q, int limiter, int k, bool pred
     if (g.act[1] && g.act[2]) {
         const unsigned int nby = (unsigned int)(((long long)g.n[0] * (g.n[1] + 1) * g.n[2] + TPB - 1) / TPB);
         const unsigned int nbz = (unsigned int)(((long long)g.n[0] * g.n[1] * (g.n[2] + 1) + TPB - 1) / TPB);
-        const dim3 nb(nby + nbz, g.nev);
+        const dim3 nb(2 * (nby > nbz ? nby : nbz), g.nev);
 #define MF_SFYZ(ST_) do { if (pred) k_sweep_flux_yz<true, ST_><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds, nby); \
                           else k_sweep_flux_yz<false, ST_><<<nb, TPB, 0, st>>>(g, q, limiter, k, V, Dl, fx, ds, nby); } while (0)
         if (g.state32) MF_SFYZ(float); else MF_SFYZ(double);
